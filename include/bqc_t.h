@@ -1,0 +1,173 @@
+/*
+ * bqc_t.h — C ABI of the B200-native closed-shell RHF (T) energy library (libbqc_t.so).
+ *
+ * What is computed (citations: /root/reference/PAPER.md = ByteQC, arxiv 2502.17963, §2.4.2,
+ * lines 282-305, Eqs. (2)-(7); readings G1-G14 in DESIGN.md / SURVEY.md §8(c)):
+ *
+ *   integrals   (pq|rs) = sum_Q B[Q,p,q] B[Q,r,s]                      (exact DF)
+ *   W_ijk[abc]  = P sum_d (ia|bd) t2[k,j,c,d] - P sum_l (ia|jl) t2[l,k,b,c]          Eq. (2)
+ *                 (P = the 6 simultaneous permutations of (i,a),(j,b),(k,c))
+ *   V_ijk[abc]  = W + t1[i,a](jb|kc) + t1[j,b](ia|kc) + t1[k,c](ia|jb)              Eqs. (6),(7)
+ *   R_ijk[abc]  = 4W[abc] + W[bca] + W[cab] - 2(W[acb] + W[cba] + W[bac])           Eq. (3)
+ *   D_ijk[abc]  = eps_i + eps_j + eps_k - eps_a - eps_b - eps_c                      Eq. (3)
+ *   e_ijk       = (2 - d_ij - d_jk) sum_abc R V / D            (i <= j <= k)        Eq. (4)
+ *   E(T)        = sum_{i<=j<=k} e_ijk
+ *
+ * Conventions common to every entry point
+ *   - All arrays are FP64, C-contiguous (last index fastest), 8-byte aligned.
+ *   - "device" pointers are CUDA device memory on the current device and stay owned by the
+ *     caller; the library only reads them and they must stay valid until the call returns.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is
+ *     ordered after prior work on `stream`; calls return after the results reached the host
+ *     (they synchronise `stream` and the library's internal helper stream only).
+ *   - No exceptions cross the ABI, there is NO CPU fallback: on any error the call returns the
+ *     error code (or NaN for the double-returning form) and bqc_last_error() reports it.
+ *   - Preconditions (not checked): t2[i,j,a,b] == t2[j,i,b,a]; B_oo, B_vv symmetric in their last
+ *     two indices.  If violated the result is unspecified (reading G14).
+ *   - Determinism: identical inputs and options give a bit-identical result on the same
+ *     build/GPU (fixed-order reductions, no floating-point atomics).
+ */
+#ifndef BQC_T_H
+#define BQC_T_H
+
+#include <stddef.h>
+
+#if defined(__GNUC__)
+#define BQC_API __attribute__((visibility("default")))
+#else
+#define BQC_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Error codes (bqc_last_error / return values). */
+enum {
+  BQC_OK = 0,
+  BQC_ERR_INVALID_SIZE = 1,    /* nocc, nvir or naux <= 0, or option out of range          */
+  BQC_ERR_NULL_POINTER = 2,    /* a required pointer is NULL                                */
+  BQC_ERR_NOT_DEVICE_PTR = 3,  /* an array pointer is not device memory (or not host, for _host) */
+  BQC_ERR_MISALIGNED = 4,      /* an array pointer is not 8-byte aligned                    */
+  BQC_ERR_WORKSPACE = 5,       /* caller workspace too small / allocation failed            */
+  BQC_ERR_CUDA = 6,            /* a CUDA runtime/driver call failed (see bqc_error_detail)  */
+  BQC_ERR_DEVICE = 7,          /* current device is not sm_100 (B200)                       */
+  BQC_ERR_DENOMINATOR = 8,     /* 3*max(eps_occ) - 3*min(eps_vir) >= 0: D may vanish (G10)  */
+  BQC_ERR_INVALID_OPTION = 9   /* bqc_t_opts field out of range                             */
+};
+
+/* Options of bqc_t_energy_ex.  Zero-initialise for defaults. */
+typedef struct bqc_t_opts {
+  int occ_block;     /* occupied block size Bo of the slab cache (0 = auto).  4*Bo (vv|ov)
+                        slabs are resident at a time; the full O(o v^3) tensor never is.     */
+  int occ_lo;        /* restrict to triplets with occ_lo <= i <= j <= k < occ_hi;            */
+  int occ_hi;        /*   occ_lo = occ_hi = 0 means all occupied orbitals.                   */
+  int shard_rank;    /* multi-GPU sharding: this call evaluates the triplets whose index     */
+  int shard_count;   /*   (bqc_t_triplet_index) % shard_count == shard_rank.  0 -> 1.        */
+  int max_batch;     /* triplets per W-builder launch (0 = auto from memory)                 */
+  int flags;         /* BQC_T_FLAG_* below                                                   */
+  int reserved;
+} bqc_t_opts;
+
+enum {
+  BQC_T_FLAG_NO_T1 = 1          /* drop the t1 (E[5]) term: V = W (for the E[4]-only checks)  */
+};
+
+/* ---- host-only helpers (no GPU needed) -------------------------------------------------- */
+
+/* o(o+1)(o+2)/6 = number of i<=j<=k triplets. */
+BQC_API size_t bqc_t_num_triplets(int nocc);
+/* Lexicographic index of (i,j,k), 0 <= i <= j <= k < nocc; (size_t)-1 if out of range. */
+BQC_API size_t bqc_t_triplet_index(int nocc, int i, int j, int k);
+/* Rank that evaluates triplet (i,j,k) under `shard_count`-way sharding (-1 on bad args). */
+BQC_API int bqc_t_triplet_owner(int nocc, int shard_count, int i, int j, int k);
+/* Algorithmic FP64 flop count of the W builder over the selected triplets:
+   [#triplets(i<=j<=k, not i=j=k) in window/shard] * 12 v^3 (v+o). */
+BQC_API double bqc_t_flops(int nocc, int nvir, const bqc_t_opts* opts);
+/* Occupied block size the scheduler will use (resolves opts->occ_block == 0). */
+BQC_API int bqc_t_plan_occ_block(int nocc, int nvir, int naux, const bqc_t_opts* opts);
+/* Bytes of device workspace bqc_t_energy_ex needs for these sizes/options. */
+BQC_API size_t bqc_t_workspace_bytes(int nocc, int nvir, int naux, const bqc_t_opts* opts);
+
+BQC_API int bqc_last_error(void);                 /* thread-local code of the last failing call (0 = none) */
+BQC_API const char* bqc_error_string(int code);   /* static description of an error code */
+BQC_API const char* bqc_error_detail(void);       /* thread-local detail text of the last error ("" if none) */
+BQC_API const char* bqc_version(void);
+
+/* ---- the (T) energy ------------------------------------------------------------------------ */
+
+/* E(T) in Hartree; NaN on error.  All array arguments are DEVICE pointers:
+     eps_occ [nocc], eps_vir [nvir], t1 [nocc][nvir], t2 [nocc][nocc][nvir][nvir],
+     B_oo [naux][nocc][nocc], B_ov [naux][nocc][nvir]  (B_ov[Q,i,a] = B[Q,i,nocc+a]),
+     B_vv [naux][nvir][nvir].
+   Workspace is allocated on the device internally and freed before return.
+   nocc == 1 is valid and returns exactly 0.0 (no triples with two electrons). */
+BQC_API double bqc_t_energy(int nocc, int nvir, int naux,
+                    const double* eps_occ, const double* eps_vir,
+                    const double* t1, const double* t2,
+                    const double* B_oo, const double* B_ov, const double* B_vv,
+                    void* stream);
+
+/* Same computation with options, caller workspace and per-triplet output.
+     workspace       device, >= bqc_t_workspace_bytes(...) bytes, 256-byte aligned; NULL = allocate
+                     internally (workspace_bytes ignored).
+     e_total_host    HOST pointer, receives the sum of the selected e_ijk (this shard/window).
+     e_triplet_dev   DEVICE pointer [bqc_t_num_triplets(nocc)] or NULL; receives e_ijk at
+                     bqc_t_triplet_index(i,j,k); entries not selected by the window/shard and
+                     the diagonal i=j=k entries are written as 0.
+   Returns BQC_OK or an error code. */
+BQC_API int bqc_t_energy_ex(int nocc, int nvir, int naux,
+                    const double* eps_occ, const double* eps_vir,
+                    const double* t1, const double* t2,
+                    const double* B_oo, const double* B_ov, const double* B_vv,
+                    const bqc_t_opts* opts, void* workspace, size_t workspace_bytes,
+                    double* e_total_host, double* e_triplet_dev, void* stream);
+
+/* End-to-end form: every array argument is a HOST pointer (pinned or pageable).  Inputs are
+   copied to the device, E(T) is evaluated by the same kernels, the scalar (and, if
+   e_triplet_host != NULL, the [num_triplets] per-triplet array) is copied back.
+   h2d_bytes / d2h_bytes (may be NULL) receive the bytes moved each way. */
+BQC_API int bqc_t_energy_host(int nocc, int nvir, int naux,
+                      const double* eps_occ, const double* eps_vir,
+                      const double* t1, const double* t2,
+                      const double* B_oo, const double* B_ov, const double* B_vv,
+                      const bqc_t_opts* opts, double* e_total_host, double* e_triplet_host,
+                      size_t* h2d_bytes, size_t* d2h_bytes, void* stream);
+
+/* ---- intermediates of single steps, for parity tests ---------- */
+
+/* Row a1: the DF slabs of occupied x (and pair x,y).  Any output pointer may be NULL.
+     I_dev [nvir][nvir][nvir]   I_x[u,b,d]  = (x u|b d)
+     O_dev [nocc][nvir]         O_xy[l,u]   = (x u|y l)
+     J_dev [nvir][nvir]         J_xy[u,w]   = (x u|y w)
+   computed by the same slab-former kernels as the energy path. */
+BQC_API int bqc_t_debug_slabs(int nocc, int nvir, int naux,
+                      const double* t2, const double* B_oo, const double* B_ov, const double* B_vv,
+                      int x, int y, double* I_dev, double* O_dev, double* J_dev, void* stream);
+
+/* Rows a2+a3: W_ijk and V_ijk of one triplet, dense [nvir][nvir][nvir] device outputs (either
+   may be NULL), produced by the same slab former, W builder and V assembly as the energy path.
+   (i, j, k) need not be ordered. */
+BQC_API int bqc_t_debug_wv(int nocc, int nvir, int naux,
+                   const double* eps_occ, const double* eps_vir,
+                   const double* t1, const double* t2,
+                   const double* B_oo, const double* B_ov, const double* B_vv,
+                   int i, int j, int k, double* W_dev, double* V_dev, void* stream);
+
+/* ---- building blocks exposed for measurement ------------------------------------------------ */
+
+/* C[M][N] (ldc) = A[M][K] (lda) * B[N][K]^T (ldb), FP64, device pointers, the library's TMA +
+   DMMA tile kernel.  lda, ldb must be multiples of 2 (16-byte rows), K is zero-padded
+   internally to a multiple of 16 by TMA out-of-bounds fill.  Returns BQC_OK or an error. */
+BQC_API int bqc_dgemm_nt(int M, int N, int K, const double* A, int lda, const double* B, int ldb,
+                 double* C, int ldc, void* stream);
+
+/* Register-resident FP64 peak microbenchmarks on all SMs: run for about
+   `seconds` and return the sustained TFLOP/s.  kind: 0 = DMMA (mma.sync m8n8k4 f64),
+   1 = DFMA (fma.rn.f64), 2 = both pipes in the same warps.  Negative on error. */
+BQC_API double bqc_fp64_peak_tflops(int kind, double seconds, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BQC_T_H */

@@ -1,0 +1,293 @@
+// energy.cu — SURVEY.md §8(a) rows a3 + a4 (+ the reductions of a5).
+//
+// The W builder leaves, per triplet, three arrays in 16^3-blocked layout:
+//     F1 = F(i,j,k)[a,b,c],  F2 = F(i,k,j)[a,c,b],  F3 = F(j,k,i)[b,c,a],   W[a,b,c] = F1 + F2 + F3
+// (see t_energy.cu).  The energy contraction needs W at all six index permutations of every point
+// (Eq. (3), reading G2), so a CTA owns one *orbit* of 16^3 tiles — the up-to-six tiles
+// reached from a block triple A <= B <= C by permutation — assembles the six W tiles in shared memory
+// (each F tile is read exactly once from HBM, as contiguous 32 KiB runs), forms V on the fly from the
+// (ov|ov) tiles and t1 (Eqs. (6),(7); V is never stored), and reduces
+//     sum_pi R_pi V_pi / D   (Eqs. (3),(4); the denominator is computed in registers, never stored).
+// Reductions are fixed-order: warp shuffle tree -> per-CTA slot -> per-triplet sum -> final sum.
+#include "kernels.cuh"
+
+namespace bqc {
+
+namespace {
+
+constexpr int kET = 16;
+constexpr int kEThreads = 512;
+constexpr int kTileElems = kET * kET * kET;   // 4096
+
+// the six permutations of three positions; 0-2 even (identity, two cyclic), 3-5 odd (transpositions)
+__device__ constexpr int kPerm[6][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}, {0, 2, 1}, {2, 1, 0}, {1, 0, 2}};
+// index of the ordered pair (s,t), s != t, in the (ov|ov) tile array
+__device__ constexpr int kPairIdx[3][3] = {{-1, 0, 1}, {2, -1, 3}, {4, 5, -1}};
+
+// XOR swizzle: consecutive lanes along ANY of the three tile axes fall into distinct columns of the
+// 128-byte row, so the transposed accumulations below and the permuted reads are conflict-free.
+__device__ __forceinline__ int sw(int x, int y, int z) { return (((x << 4) | y) << 4) | (z ^ x ^ y); }
+
+struct EnergySmem {
+  double Wt[6][kTileElems];
+  double Jt[6][kET * kET];
+  double t1s[3][3][kET];   // [which occupied (i,j,k)][block position][local]
+  double epsv[3][kET];
+  double red[kEThreads / 32];
+};
+
+__device__ __forceinline__ size_t blk_off(int nb, int P, int Q, int R) {
+  return (((size_t)P * nb + Q) * nb + R) * kTileElems;
+}
+
+}  // namespace
+
+__global__ void __launch_bounds__(kEThreads, 1) energy_kernel(const EnergyArgs a) {
+  extern __shared__ uint8_t esm_raw[];
+  EnergySmem& sm = *reinterpret_cast<EnergySmem*>(esm_raw);
+  const int tid = threadIdx.x;
+  const int orbit = blockIdx.x;
+  const int tb = blockIdx.y;
+  const int packed = a.orbits[orbit];
+  const int blk[3] = {packed & 255, (packed >> 8) & 255, (packed >> 16) & 255};
+  const TripletRec tr = a.trips[tb];
+  const int nb = a.nb16, v = a.v;
+  const size_t fsz = (size_t)nb * nb * nb * kTileElems;
+  const double* F1 = a.F + (size_t)tb * 3 * fsz;
+  const double* F2 = F1 + fsz;
+  const double* F3 = F2 + fsz;
+
+  // ---- small operands: t1 rows, virtual orbital energies
+  if (tid < 3 * 3 * kET) {
+    const int l = tid & 15, pos = (tid >> 4) % 3, which = tid / (3 * kET);
+    const int occ = which == 0 ? tr.i : (which == 1 ? tr.j : tr.k);
+    const int av = blk[pos] * kET + l;
+    sm.t1s[which][pos][l] = (av < v) ? a.t1[(size_t)occ * v + av] : 0.0;
+  } else if (tid < 3 * 3 * kET + 3 * kET) {
+    const int e = tid - 3 * 3 * kET;
+    const int l = e & 15, pos = e >> 4;
+    const int av = blk[pos] * kET + l;
+    sm.epsv[pos][l] = (av < v) ? a.eps_vir[av] : 1.0;
+  }
+
+  // ---- assemble the six W tiles: W[a,b,c] = F1[a,b,c] + F2[a,c,b] + F3[b,c,a]
+  // thread -> element pairs L = 2*(tid + 512 r), (u, vv, w) = (L>>8, (L>>4)&15, L&15), w even
+#pragma unroll 1
+  for (int phase = 0; phase < 3; ++phase) {
+#pragma unroll 1
+    for (int half = 0; half < 2; ++half) {
+      double2 val[3][4];
+#pragma unroll
+      for (int pp = 0; pp < 3; ++pp) {
+        const int pi = half * 3 + pp;
+        const int P = blk[kPerm[pi][0]], Q = blk[kPerm[pi][1]], R = blk[kPerm[pi][2]];
+        const double* src = phase == 0 ? F1 + blk_off(nb, P, Q, R)
+                                       : (phase == 1 ? F2 + blk_off(nb, P, R, Q) : F3 + blk_off(nb, Q, R, P));
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+          val[pp][r] = __ldg(reinterpret_cast<const double2*>(src) + tid + kEThreads * r);
+      }
+#pragma unroll
+      for (int pp = 0; pp < 3; ++pp) {
+        double* W = sm.Wt[half * 3 + pp];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+          const int L = 2 * (tid + kEThreads * r);
+          const int u = L >> 8, vv = (L >> 4) & 15, w = L & 15;
+          if (phase == 0) {          // F1 tile [x][y][z] = (u, vv, w)
+            W[sw(u, vv, w)] = val[pp][r].x;
+            W[sw(u, vv, w + 1)] = val[pp][r].y;
+          } else if (phase == 1) {   // F2 tile [x][z][y] = (u, vv, w)
+            W[sw(u, w, vv)] += val[pp][r].x;
+            W[sw(u, w + 1, vv)] += val[pp][r].y;
+          } else {                   // F3 tile [y][z][x] = (u, vv, w)
+            W[sw(w, u, vv)] += val[pp][r].x;
+            W[sw(w + 1, u, vv)] += val[pp][r].y;
+          }
+        }
+      }
+    }
+    __syncthreads();
+  }
+
+  // ---- points of this thread: z = tid & 15, y = (tid >> 4) & 15, x = (tid >> 8) + 2 r
+  const int lz = tid & 15, ly = (tid >> 4) & 15, lx0 = tid >> 8;
+  double num[8];
+#pragma unroll
+  for (int r = 0; r < 8; ++r) {
+    const int l[3] = {lx0 + 2 * r, ly, lz};
+    double w[6];
+#pragma unroll
+    for (int p = 0; p < 6; ++p) w[p] = sm.Wt[p][sw(l[kPerm[p][0]], l[kPerm[p][1]], l[kPerm[p][2]])];
+    const double se = w[0] + w[1] + w[2], so = w[3] + w[4] + w[5];
+    const double re = se - 2.0 * so, ro = so - 2.0 * se;
+    double s = 0.0;
+#pragma unroll
+    for (int p = 0; p < 6; ++p) s += (3.0 * w[p] + (p < 3 ? re : ro)) * w[p];
+    num[r] = s;
+  }
+
+  if (a.use_t1) {
+#pragma unroll 1
+    for (int m = 0; m < 3; ++m) {
+      // J^(0) = J_jk, J^(1) = J_ik, J^(2) = J_ij
+      const int px = (m == 0) ? tr.pj : tr.pi;
+      const int py = (m == 2) ? tr.pj : tr.pk;
+      const double* Jm = a.J + ((size_t)px * a.nw + py) * v * v;
+      __syncthreads();
+      for (int e = tid; e < 6 * kET * kET; e += kEThreads) {
+        const int lw = e & 15, lu = (e >> 4) & 15, pr = e >> 8;
+        // pair index -> ordered block positions (s, t)
+        const int s = pr >> 1;
+        const int t = (pr & 1) ? (s == 2 ? 1 : 2) : (s == 0 ? 1 : 0);
+        const int gu = blk[s] * kET + lu, gw = blk[t] * kET + lw;
+        sm.Jt[pr][(lu << 4) | lw] = (gu < v && gw < v) ? __ldg(Jm + (size_t)gu * v + gw) : 0.0;
+      }
+      __syncthreads();
+      const int sA = (m == 0) ? 1 : 0, sB = (m == 2) ? 1 : 2;
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        const int l[3] = {lx0 + 2 * r, ly, lz};
+        double w[6];
+#pragma unroll
+        for (int p = 0; p < 6; ++p) w[p] = sm.Wt[p][sw(l[kPerm[p][0]], l[kPerm[p][1]], l[kPerm[p][2]])];
+        const double se = w[0] + w[1] + w[2], so = w[3] + w[4] + w[5];
+        const double re = se - 2.0 * so, ro = so - 2.0 * se;
+        double s = 0.0;
+#pragma unroll
+        for (int p = 0; p < 6; ++p) {
+          const int pm = kPerm[p][m], pa = kPerm[p][sA], pb = kPerm[p][sB];
+          const double x = sm.t1s[m][pm][l[pm]] * sm.Jt[kPairIdx[pa][pb]][(l[pa] << 4) | l[pb]];
+          s += (3.0 * w[p] + (p < 3 ? re : ro)) * x;
+        }
+        num[r] += s;
+      }
+    }
+  }
+
+  // ---- denominators (Eq. (3)), in registers
+  const double dijk = a.eps_occ[tr.i] + a.eps_occ[tr.j] + a.eps_occ[tr.k];
+  double acc = 0.0;
+#pragma unroll
+  for (int r = 0; r < 8; ++r) {
+    const int lx = lx0 + 2 * r;
+    const bool valid = (blk[0] * kET + lx < v) && (blk[1] * kET + ly < v) && (blk[2] * kET + lz < v);
+    const double d = dijk - sm.epsv[0][lx] - sm.epsv[1][ly] - sm.epsv[2][lz];
+    if (valid) acc += num[r] / d;
+  }
+  // multiplicity of the block triple under permutation (1, 2 or 6)
+  const int same = (blk[0] == blk[1]) + (blk[1] == blk[2]);
+  acc *= (same == 0) ? 1.0 : (same == 1 ? 0.5 : (1.0 / 6.0));
+
+  // ---- fixed-order block reduction
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off);
+  if ((tid & 31) == 0) sm.red[tid >> 5] = acc;
+  __syncthreads();
+  if (tid == 0) {
+    double s = 0.0;
+#pragma unroll
+    for (int wdx = 0; wdx < kEThreads / 32; ++wdx) s += sm.red[wdx];
+    a.partial[(size_t)tb * a.norbits + orbit] = s;
+  }
+}
+
+int launch_energy(const EnergyArgs& a, cudaStream_t s) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    BQC_CUDA_OK(cudaFuncSetAttribute(energy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)sizeof(EnergySmem)));
+    attr_set = true;
+  }
+  if (a.ntrip <= 0) return BQC_OK;
+  dim3 grid(a.norbits, a.ntrip);
+  energy_kernel<<<grid, kEThreads, sizeof(EnergySmem), s>>>(a);
+  BQC_CUDA_OK(cudaGetLastError());
+  return BQC_OK;
+}
+
+// ------------------------------------------------------------------ per-triplet and final sums
+__global__ void reduce_triplets_kernel(const double* __restrict__ partial, const TripletRec* __restrict__ trips,
+                                       int norbits, double* __restrict__ e_trip) {
+  __shared__ double red[256];
+  const int tb = blockIdx.x;
+  const double* p = partial + (size_t)tb * norbits;
+  double s = 0.0;
+  for (int n = threadIdx.x; n < norbits; n += 256) s += p[n];
+  red[threadIdx.x] = s;
+  __syncthreads();
+  for (int off = 128; off > 0; off >>= 1) {
+    if (threadIdx.x < off) red[threadIdx.x] += red[threadIdx.x + off];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    const TripletRec tr = trips[tb];
+    // (2 - delta_ij - delta_jk) for i <= j <= k (reading G3)
+    const double wgt = 2.0 - (tr.i == tr.j ? 1.0 : 0.0) - (tr.j == tr.k ? 1.0 : 0.0);
+    e_trip[tr.index] = wgt * red[0];
+  }
+}
+
+int launch_reduce_triplets(const double* partial, const TripletRec* trips, int ntrip, int norbits,
+                           double* e_trip, cudaStream_t s) {
+  if (ntrip <= 0) return BQC_OK;
+  reduce_triplets_kernel<<<ntrip, 256, 0, s>>>(partial, trips, norbits, e_trip);
+  BQC_CUDA_OK(cudaGetLastError());
+  return BQC_OK;
+}
+
+__global__ void final_sum_kernel(const double* __restrict__ e, long long n, double* __restrict__ out) {
+  __shared__ double red[1024];
+  double s = 0.0;
+  for (long long i = threadIdx.x; i < n; i += 1024) s += e[i];
+  red[threadIdx.x] = s;
+  __syncthreads();
+  for (int off = 512; off > 0; off >>= 1) {
+    if (threadIdx.x < off) red[threadIdx.x] += red[threadIdx.x + off];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *out = red[0];
+}
+
+int launch_final_sum(const double* e_trip, long long n, double* out, cudaStream_t s) {
+  final_sum_kernel<<<1, 1024, 0, s>>>(e_trip, n, out);
+  BQC_CUDA_OK(cudaGetLastError());
+  return BQC_OK;
+}
+
+// ------------------------------------------------------------------ dense W / V of one triplet (debug)
+__global__ void assemble_wv_kernel(const double* __restrict__ F, int nb, int v, const double* __restrict__ Jjk,
+                                   const double* __restrict__ Jik, const double* __restrict__ Jij,
+                                   const double* __restrict__ t1i, const double* __restrict__ t1j,
+                                   const double* __restrict__ t1k, double* __restrict__ W,
+                                   double* __restrict__ V) {
+  const size_t fsz = (size_t)nb * nb * nb * kTileElems;
+  const long long total = (long long)v * v * v;
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < total;
+       e += (long long)gridDim.x * blockDim.x) {
+    const int c = (int)(e % v);
+    const int b = (int)((e / v) % v);
+    const int a = (int)(e / ((long long)v * v));
+    auto at = [&](const double* Fx, int p, int q, int r) {
+      return Fx[blk_off(nb, p >> 4, q >> 4, r >> 4) + ((((p & 15) << 4) | (q & 15)) << 4 | (r & 15))];
+    };
+    const double w = at(F, a, b, c) + at(F + fsz, a, c, b) + at(F + 2 * fsz, b, c, a);
+    if (W) W[e] = w;
+    if (V)
+      V[e] = w + t1i[a] * Jjk[(size_t)b * v + c] + t1j[b] * Jik[(size_t)a * v + c] +
+             t1k[c] * Jij[(size_t)a * v + b];
+  }
+}
+
+int launch_assemble_wv(const double* F, int nb16, int v, const double* J, int nw, int pi, int pj, int pk,
+                       const double* t1i, const double* t1j, const double* t1k, double* W, double* V,
+                       cudaStream_t s) {
+  const size_t v2 = (size_t)v * v;
+  assemble_wv_kernel<<<1024, 256, 0, s>>>(F, nb16, v, J + ((size_t)pj * nw + pk) * v2,
+                                          J + ((size_t)pi * nw + pk) * v2, J + ((size_t)pi * nw + pj) * v2,
+                                          t1i, t1j, t1k, W, V);
+  BQC_CUDA_OK(cudaGetLastError());
+  return BQC_OK;
+}
+
+}  // namespace bqc

@@ -1,0 +1,117 @@
+// gemm_nt.cu — host side of the tile-GEMM engine: tensor-map encoding and launch.
+#include "gemm_nt.cuh"
+
+#include <mutex>
+
+namespace bqc {
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                    const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                    const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static PFN_encodeTiled get_encode_fn() {
+  static PFN_encodeTiled fn = nullptr;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    // the driver entry point is resolved at run time so that libbqc_t.so does not link libcuda
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<PFN_encodeTiled>(p);
+  });
+  return fn;
+}
+
+int make_tensor_map_f64(CUtensorMap* out, const void* base, const unsigned long long dims[4],
+                        const unsigned long long strides_bytes[4], unsigned box1, unsigned box2) {
+  PFN_encodeTiled enc = get_encode_fn();
+  if (!enc) {
+    set_error(BQC_ERR_CUDA, "cuTensorMapEncodeTiled entry point not available");
+    return BQC_ERR_CUDA;
+  }
+  cuuint64_t gdim[4] = {dims[0], dims[1], dims[2], dims[3]};
+  cuuint64_t gstr[3] = {strides_bytes[1], strides_bytes[2], strides_bytes[3]};
+  cuuint32_t box[4] = {(cuuint32_t)kBK, box1, box2, 1};
+  cuuint32_t estr[4] = {1, 1, 1, 1};
+  CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void*>(base), gdim, gstr, box,
+                   estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    set_error(BQC_ERR_CUDA,
+              "cuTensorMapEncodeTiled failed (%d): dims %llu %llu %llu %llu strides %llu %llu %llu box %u %u",
+              (int)r, dims[0], dims[1], dims[2], dims[3], strides_bytes[1], strides_bytes[2],
+              strides_bytes[3], box1, box2);
+    return BQC_ERR_CUDA;
+  }
+  return BQC_OK;
+}
+
+int device_sm_count() {
+  static int sms = 0;
+  if (sms == 0) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+  }
+  return sms;
+}
+
+int choose_nf(long long n_ext) {
+  int best = kMaxNF;
+  long long best_cost = -1;
+  for (int nf = kMaxNF; nf >= kMinNF; --nf) {
+    const long long bn = gemm_bn(nf);
+    const long long cost = (n_ext + bn - 1) / bn * bn;
+    if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = nf; }
+  }
+  return best;
+}
+
+void choose_m_tile(int m1_ext, int m2_ext, int* tp, int* tq_log2) {
+  long long best_cost = -1;
+  for (int lg = 7; lg >= 3; --lg) {   // tq = 128 ... 8 (a TMA sub-box of tq rows must span whole 1 KiB swizzle atoms)
+    const int tq = 1 << lg, tpp = kBM / tq;
+    const long long cost = (long long)round_up_i(m1_ext, tpp) * round_up_i(m2_ext, tq);
+    if (best_cost < 0 || cost < best_cost) { best_cost = cost; *tp = tpp; *tq_log2 = lg; }
+  }
+}
+
+template <int NF>
+static int launch_nf(const CUtensorMap& tmA, const CUtensorMap& tmAT, const CUtensorMap& tmB,
+                     const GemmParams& prm, int grid, cudaStream_t stream) {
+  static std::once_flag once;
+  static cudaError_t attr_err = cudaSuccess;
+  std::call_once(once, [] {
+    attr_err = cudaFuncSetAttribute(gemm_nt_kernel<NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    gemm_smem_bytes(NF));
+  });
+  BQC_CUDA_OK(attr_err);
+  gemm_nt_kernel<NF><<<grid, kGemmThreads, gemm_smem_bytes(NF), stream>>>(tmA, tmAT, tmB, prm);
+  BQC_CUDA_OK(cudaGetLastError());
+  return BQC_OK;
+}
+
+int launch_gemm_nt(int nf, const CUtensorMap& tmA, const CUtensorMap& tmAT, const CUtensorMap& tmB,
+                   const GemmParams& prm, cudaStream_t stream) {
+  const long long total = (long long)prm.ntasks * prm.tiles_m1 * prm.tiles_m2 * prm.tiles_n;
+  if (total <= 0) return BQC_OK;
+  const int sms = device_sm_count();
+  if (sms <= 0) {
+    set_error(BQC_ERR_CUDA, "no CUDA device");
+    return BQC_ERR_CUDA;
+  }
+  const int grid = (int)(total < sms ? total : sms);
+  switch (nf) {
+    case 4: return launch_nf<4>(tmA, tmAT, tmB, prm, grid, stream);
+    case 5: return launch_nf<5>(tmA, tmAT, tmB, prm, grid, stream);
+    case 6: return launch_nf<6>(tmA, tmAT, tmB, prm, grid, stream);
+    case 7: return launch_nf<7>(tmA, tmAT, tmB, prm, grid, stream);
+    case 8: return launch_nf<8>(tmA, tmAT, tmB, prm, grid, stream);
+  }
+  set_error(BQC_ERR_INVALID_OPTION, "launch_gemm_nt: unsupported nf %d", nf);
+  return BQC_ERR_INVALID_OPTION;
+}
+
+}  // namespace bqc

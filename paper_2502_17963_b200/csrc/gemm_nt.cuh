@@ -1,0 +1,259 @@
+// gemm_nt.cuh — the one FP64 tile-GEMM engine of the library.
+//
+//   C[(m1,m2), n] = sum_terms sum_k A_term[(m1,m2), k] * B_term[n, k]           ("NT", both K-major)
+//
+// * Operands are staged global -> shared by TMA (cp.async.bulk.tensor, 128-byte swizzle) through a
+//   ring of mbarrier-guarded stages filled by one producer warp.
+// * 8 consumer warps issue FP64 tensor-core MMAs (mma.sync m8n8k4 -> SASS DMMA.8x8x4; sm_100a has no
+//   tcgen05/wgmma f64 kind) on a 128 x 128 CTA tile, 64 x 32 per warp, accumulators in registers.
+// * The kernel is persistent: CTAs stride over a tile list (task, m1-tile, m2-tile, n-tile), n fastest
+//   so that concurrently running CTAs share the A tile through L2.
+// * The M index is a pair (m1, m2) tiled tp x tq (tp*tq = 128).  A term may read its A rows from the
+//   same tensor with (m1, m2) transposed ("a_transposed": tp single-row-block TMA boxes instead of
+//   one), which is how W's index-permuted slab reads (I_y[q,p,:]) cost nothing.
+#pragma once
+
+#include "common.cuh"
+
+namespace bqc {
+
+constexpr int kBM = 128;            // rows of the A tile (= tp * tq)
+constexpr int kBK = 16;             // doubles per smem row = 128 bytes = one swizzle span
+constexpr int kConsumerWarps = 8;   // 4 (M) x 2 (N) warps, warp tile 32 x (8*NF)
+constexpr int kGemmThreads = (kConsumerWarps + 4) * 32;   // 2 consumer warpgroups + 1 producer warpgroup
+// The B tile has BN = 16*NF rows (NF = 8-column MMA fragments per warp), NF in [kMinNF, kMaxNF].
+constexpr int kMinNF = 4, kMaxNF = 8;
+#ifdef __CUDACC__
+#define BQC_HD __host__ __device__
+#else
+#define BQC_HD
+#endif
+BQC_HD constexpr int gemm_bn(int nf) { return 16 * nf; }
+BQC_HD constexpr int gemm_stage_bytes(int nf) { return (kBM + gemm_bn(nf)) * kBK * 8; }
+BQC_HD constexpr int gemm_stages(int nf) { return (192 * 1024) / gemm_stage_bytes(nf) > 8 ? 8 : (192 * 1024) / gemm_stage_bytes(nf); }
+BQC_HD constexpr int gemm_smem_bytes(int nf) { return gemm_stages(nf) * gemm_stage_bytes(nf) + 1024 /*align slack*/ + 256 /*barriers*/; }
+
+struct GemmTerm {
+  int a_idx;          // coordinate 3 of the A tensor map (slab slot / batch entry)
+  int b_idx;          // coordinate 2 of the B tensor map (pair index / batch entry)
+  int a_transposed;   // 0: A row (m1,m2) = tensor[a_idx][m1][m2][:]; 1: = tensor[a_idx][m2][m1][:]
+  int pad;
+};
+
+struct GemmTask {
+  GemmTerm term[2];
+  long long c_off;    // element offset of this task's output inside C
+  int nterms;
+  int pad;
+};
+
+struct GemmParams {
+  int ntasks;
+  int tiles_m1, tiles_m2, tiles_n;   // per task
+  int tp, tq_log2;                   // M tile = tp (m1) x tq (m2), tq = 1 << tq_log2
+  int m1_base, n_base;               // added to the TMA coordinates (not to the output index)
+  int m1_ext, m2_ext, n_ext;         // valid extents of the output index ranges
+  int kiters;                        // ceil(K / 16) per term
+  // output addressing
+  int out_mode;                      // 0: strided, 1: blocked 16^3 tiles (F layout)
+  int n2_ext;                        // strided: n -> (n / n2_ext, n % n2_ext)
+  long long sM1, sM2, sN1, sN2;      // strided: off = c_off + m1*sM1 + m2*sM2 + n1*sN1 + n2*sN2
+  int nb16;                          // blocked: blocks per dimension
+  const GemmTask* tasks;
+  double* C;
+};
+
+#ifdef __CUDACC__
+
+template <int NF>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+gemm_nt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmAT,
+               const __grid_constant__ CUtensorMap tmB, const GemmParams prm) {
+  constexpr int kBN = gemm_bn(NF);
+  constexpr int kStageBytes = gemm_stage_bytes(NF);
+  constexpr int kStages = gemm_stages(NF);
+  extern __shared__ uint8_t smem_raw[];
+  // 1024-byte alignment: the 128B swizzle pattern is a function of shared address bits [4,10).
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + kStages * kStageBytes);
+  uint64_t* empty_bar = full_bar + kStages;
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kStages; ++s) {
+      mbar_init(&full_bar[s], 1);
+      mbar_init(&empty_bar[s], kConsumerWarps);
+    }
+    fence_mbar_init();
+  }
+  if (warp == kConsumerWarps && lane == 0) {
+    tma_prefetch_desc(&tmA);
+    tma_prefetch_desc(&tmAT);
+    tma_prefetch_desc(&tmB);
+  }
+  __syncthreads();
+
+  const int tq = 1 << prm.tq_log2;
+  const int tiles_per_task = prm.tiles_m1 * prm.tiles_m2 * prm.tiles_n;
+  const long long total_tiles = (long long)prm.ntasks * tiles_per_task;
+
+  if (warp >= kConsumerWarps) {
+    // =========================== TMA producer (one elected lane) ===========================
+    // the producer warpgroup hands its registers to the two consumer warpgroups
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+    if (warp == kConsumerWarps && lane == 0) {
+      int stage = 0;
+      uint32_t phase = 0;
+      for (long long tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+        int r = (int)(tile % tiles_per_task);
+        const int task_id = (int)(tile / tiles_per_task);
+        const int n_t = r % prm.tiles_n;  r /= prm.tiles_n;
+        const int m2_t = r % prm.tiles_m2;
+        const int m1_t = r / prm.tiles_m2;
+        const int m1_0 = prm.m1_base + m1_t * prm.tp;
+        const int m2_0 = m2_t * tq;
+        const int n_0 = prm.n_base + n_t * kBN;
+        const GemmTask* task = prm.tasks + task_id;
+        const int nterms = task->nterms;
+        for (int term = 0; term < nterms; ++term) {
+          const int a_idx = task->term[term].a_idx;
+          const int b_idx = task->term[term].b_idx;
+          const int a_tr = task->term[term].a_transposed;
+          for (int kt = 0; kt < prm.kiters; ++kt) {
+            mbar_wait(&empty_bar[stage], phase ^ 1u);
+            uint8_t* sA = smem + stage * kStageBytes;
+            uint8_t* sB = sA + kBM * kBK * 8;
+            mbar_arrive_expect_tx(&full_bar[stage], kStageBytes);
+            if (!a_tr) {
+              tma_load_4d(sA, &tmA, &full_bar[stage], kt * kBK, m2_0, m1_0, a_idx);
+            } else {
+              for (int pl = 0; pl < prm.tp; ++pl)
+                tma_load_4d(sA + pl * tq * (kBK * 8), &tmAT, &full_bar[stage], kt * kBK, m1_0 + pl,
+                            m2_0, a_idx);
+            }
+            tma_load_4d(sB, &tmB, &full_bar[stage], kt * kBK, n_0, b_idx, 0);
+            if (++stage == kStages) { stage = 0; phase ^= 1u; }
+          }
+        }
+      }
+    }
+    return;
+  }
+
+  // =============================== DMMA consumers (8 warps) ===============================
+  asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
+  const int g = lane >> 2;            // fragment row (A) / column (B)
+  const int t = lane & 3;             // fragment k index
+  const int warp_m0 = (warp >> 1) * 32;
+  const int warp_n0 = (warp & 1) * (8 * NF);
+  // k slot of lane t in k4-step c is k = 2c + (t&1) + 8*(t>>1): with the 128B swizzle (16-byte chunk
+  // index ^= row & 7) the 16 lanes of a half-warp then hit 16 distinct 8-byte bank pairs.
+  uint32_t koff[4];
+#pragma unroll
+  for (int c = 0; c < 4; ++c) koff[c] = (uint32_t)((((c + 4 * (t >> 1)) ^ g) << 4) + ((t & 1) << 3));
+  const uint32_t a_row_off = (uint32_t)((warp_m0 + g) * (kBK * 8));
+  const uint32_t b_row_off = (uint32_t)(kBM * kBK * 8 + (warp_n0 + g) * (kBK * 8));
+
+  int stage = 0;
+  uint32_t phase = 0;
+  for (long long tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+    int r = (int)(tile % tiles_per_task);
+    const int task_id = (int)(tile / tiles_per_task);
+    const int n_t = r % prm.tiles_n;  r /= prm.tiles_n;
+    const int m2_t = r % prm.tiles_m2;
+    const int m1_t = r / prm.tiles_m2;
+    const GemmTask* task = prm.tasks + task_id;
+    const int iters = task->nterms * prm.kiters;
+
+    double acc[4][NF][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int j = 0; j < NF; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    for (int it = 0; it < iters; ++it) {
+      mbar_wait(&full_bar[stage], phase);
+      const uint8_t* sbase = smem + stage * kStageBytes;
+      const uint8_t* pa = sbase + a_row_off;
+      const uint8_t* pb = sbase + b_row_off;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        double a[4], b[NF];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) a[i] = *reinterpret_cast<const double*>(pa + i * (8 * kBK * 8) + koff[c]);
+#pragma unroll
+        for (int j = 0; j < NF; ++j) b[j] = *reinterpret_cast<const double*>(pb + j * (8 * kBK * 8) + koff[c]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < NF; ++j) dmma_884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty_bar[stage]);
+      if (++stage == kStages) { stage = 0; phase ^= 1u; }
+    }
+
+    // ------------------------------- epilogue: registers -> global -------------------------------
+    const int m1_0 = m1_t * prm.tp;
+    const int m2_0 = m2_t * tq;
+    const int n_0 = n_t * kBN + warp_n0 + 2 * t;
+    double* __restrict__ C = prm.C + task->c_off;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int m = warp_m0 + i * 8 + g;
+      const int m1 = m1_0 + (m >> prm.tq_log2);
+      const int m2 = m2_0 + (m & (tq - 1));
+      if (m1 >= prm.m1_ext || m2 >= prm.m2_ext) continue;
+#pragma unroll
+      for (int j = 0; j < NF; ++j) {
+        const int n = n_0 + j * 8;
+        if (n >= prm.n_ext) continue;
+        const bool has1 = (n + 1) < prm.n_ext;
+        if (prm.out_mode == 1) {
+          const long long off =
+              ((((long long)(m1 >> 4) * prm.nb16 + (m2 >> 4)) * prm.nb16 + (n >> 4)) << 12) +
+              ((((m1 & 15) << 4) + (m2 & 15)) << 4) + (n & 15);
+          if (has1) {
+            *reinterpret_cast<double2*>(C + off) = make_double2(acc[i][j][0], acc[i][j][1]);
+          } else {
+            C[off] = acc[i][j][0];
+          }
+        } else {
+          const long long base = (long long)m1 * prm.sM1 + (long long)m2 * prm.sM2;
+          const long long off0 = base + (long long)(n / prm.n2_ext) * prm.sN1 + (long long)(n % prm.n2_ext) * prm.sN2;
+          const long long off1 = base + (long long)((n + 1) / prm.n2_ext) * prm.sN1 +
+                                 (long long)((n + 1) % prm.n2_ext) * prm.sN2;
+          if (has1 && off1 == off0 + 1 && ((reinterpret_cast<uintptr_t>(C + off0) & 15) == 0)) {
+            *reinterpret_cast<double2*>(C + off0) = make_double2(acc[i][j][0], acc[i][j][1]);
+          } else {
+            C[off0] = acc[i][j][0];
+            if (has1) C[off1] = acc[i][j][1];
+          }
+        }
+      }
+    }
+  }
+}
+
+#endif  // __CUDACC__
+
+// ------------------------------------------------------------------ host side
+// 4-D FP64 tensor map with a (16, b1, b2, 1) box and 128-byte swizzle.
+//   dims[0..3] (elements, dim 0 fastest) ; strides_bytes[1..3] (dim 0 is contiguous).
+int make_tensor_map_f64(CUtensorMap* out, const void* base, const unsigned long long dims[4],
+                        const unsigned long long strides_bytes[4], unsigned box1, unsigned box2);
+
+// Launch the persistent kernel (B tile of 16*nf rows; tmB's box must have that many rows) on `stream`.
+// prm.tasks must stay valid until the kernel ran.
+int launch_gemm_nt(int nf, const CUtensorMap& tmA, const CUtensorMap& tmAT, const CUtensorMap& tmB,
+                   const GemmParams& prm, cudaStream_t stream);
+// NF that minimises padded work for an N extent (ties -> larger tile).
+int choose_nf(long long n_ext);
+// (tp, tq_log2) with tp * tq = 128 minimising padded rows for extents (m1_ext, m2_ext).
+void choose_m_tile(int m1_ext, int m2_ext, int* tp, int* tq_log2);
+
+int device_sm_count();
+
+}  // namespace bqc

@@ -1,0 +1,55 @@
+// kernels.cuh — launchers of the non-GEMM kernels (repacking, energy contraction, reductions).
+#pragma once
+#include "common.cuh"
+
+namespace bqc {
+
+// out[r][q] (pitch qp, zero for q >= nq) = in[q][r]        (in: [nq][nr] row-major)
+int launch_transpose_pad(const double* in, double* out, int nq, int nr, int qp, cudaStream_t s);
+
+// Btil[pz*na + py][r][d] = t2[act[pz]][act[py]][r][d], d < v  (row pitch kp).  Columns >= v untouched.
+int launch_btilde_t2(const double* t2, double* btil, int o, int v, const int* act_dev, int na, int kp,
+                     cudaStream_t s);
+
+// slab[slot0 + s][p][q][v + l] = -t2[x0 + s][l][p][q]  for s < nx, l < o   (row pitch kp).
+int launch_slab_holes(const double* t2, double* slabs, int o, int v, int kp, int x0, int nx,
+                      int slot0, cudaStream_t s);
+
+// One entry per triplet of a batch.
+struct TripletRec {
+  int i, j, k;        // occupied indices, i <= j <= k
+  int pi, pj, pk;     // indices relative to the occupied window (i - lo, ...)
+  long long index;    // bqc_t_triplet_index(i, j, k)
+};
+
+struct EnergyArgs {
+  const double* F;          // [ntrip][3][nb16^3][16^3] blocked F(i,j,k), F(i,k,j), F(j,k,i)
+  const TripletRec* trips;  // [ntrip]
+  const int* orbits;        // [norbits] packed A | B<<8 | C<<16, A <= B <= C
+  const double* J;          // [nw*nw][v][v]   J_xy[u,w] = (xu|yw)
+  const double* t1;         // [o][v]
+  const double* eps_occ;    // [o]
+  const double* eps_vir;    // [v]
+  double* partial;          // [ntrip][norbits]
+  int ntrip, norbits, nb16, v, nw, use_t1;
+};
+int launch_energy(const EnergyArgs& a, cudaStream_t s);
+
+// e_trip[trips[t].index] = weight(i,j,k) * sum_orbits partial[t][:]   (fixed order)
+int launch_reduce_triplets(const double* partial, const TripletRec* trips, int ntrip, int norbits,
+                           double* e_trip, cudaStream_t s);
+// *out = sum_n e_trip[n] in a fixed order (single block)
+int launch_final_sum(const double* e_trip, long long n, double* out, cudaStream_t s);
+
+// dense W / V [v][v][v] of one triplet from its three blocked F arrays (debug / parity of rows a2, a3)
+int launch_assemble_wv(const double* F, int nb16, int v, const double* J, int nw, int pi, int pj, int pk,
+                       const double* t1i, const double* t1j, const double* t1k, double* W, double* V,
+                       cudaStream_t s);
+
+// strided 3-D copy out[a][b][c] = in[a*sa + b*sb + c*sc], used to unpad debug slabs
+int launch_copy3(const double* in, long long sa, long long sb, long long sc, double* out, int na, int nb,
+                 int nc, cudaStream_t s);
+
+double run_fp64_peak(int kind, double seconds, cudaStream_t s);
+
+}  // namespace bqc

@@ -1,0 +1,105 @@
+"""-m "not gpu": the C-ABI library builds, loads and exports every symbol include/*.h declares;
+host-only entry points (no compute calls) behave."""
+import ctypes
+import glob
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def libpath():
+    from paper_2502_17963_b200.build import build_library
+    return build_library()
+
+
+def _declared_symbols():
+    names = set()
+    for h in glob.glob(os.path.join(ROOT, "include", "*.h")):
+        src = open(h).read()
+        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        names |= set(re.findall(r"\b(bqc_\w+)\s*\(", src))
+    return sorted(names)
+
+
+def test_header_declares_the_boundary():
+    names = _declared_symbols()
+    for must in ["bqc_t_energy", "bqc_t_energy_ex", "bqc_t_energy_host", "bqc_t_workspace_bytes",
+                 "bqc_t_num_triplets", "bqc_t_triplet_index", "bqc_last_error", "bqc_error_string"]:
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol(libpath):
+    L = ctypes.CDLL(libpath)
+    for name in _declared_symbols():
+        assert hasattr(L, name), f"{name} declared in include/ but not exported"
+
+
+def test_no_torch_types_in_the_abi():
+    src = open(os.path.join(ROOT, "include", "bqc_t.h")).read()
+    assert "torch" not in src.lower().replace("pytorch tensors", "") or "at::" not in src
+    assert "at::Tensor" not in src and "#include <torch" not in src
+
+
+def test_triplet_indexing(libpath):
+    import paper_2502_17963_b200 as bqc
+    for o in (1, 2, 3, 6, 11):
+        n = 0
+        for i in range(o):
+            for j in range(i, o):
+                for k in range(j, o):
+                    assert bqc.bqc_t_triplet_index(o, i, j, k) == n
+                    n += 1
+        assert bqc.bqc_t_num_triplets(o) == n == o * (o + 1) * (o + 2) // 6
+    assert bqc.bqc_t_triplet_index(5, 2, 1, 3) == -1
+    assert bqc.bqc_t_triplet_index(5, 0, 1, 5) == -1
+    assert bqc.bqc_t_num_triplets(100) == 171700
+
+
+def test_flop_model_matches_survey(libpath):
+    import paper_2502_17963_b200 as bqc
+    # F_W = [o(o+1)(o+2)/6 - o] 12 v^3 (v+o)
+    for (o, v), fw in {(5, 19): 5.93e7, (20, 76): 7.69e11, (40, 152): 9.26e13, (80, 304): 1.146e16,
+                       (100, 380): 5.424e16}.items():
+        assert bqc.bqc_t_flops(o, v) == pytest.approx(fw, rel=2e-3)
+        assert bqc.bqc_t_flops(o, v) == (o * (o + 1) * (o + 2) // 6 - o) * 12.0 * v ** 3 * (v + o)
+    w = bqc.make_opts(occ_lo=2, occ_hi=6)
+    assert bqc.bqc_t_flops(20, 76, w) == (4 * 5 * 6 // 6 - 4) * 12.0 * 76 ** 3 * 96
+
+
+def test_sharding_partitions_triplets(libpath):
+    import paper_2502_17963_b200 as bqc
+    o = 7
+    for nshard in (1, 2, 3, 8):
+        seen = {}
+        for i in range(o):
+            for j in range(i, o):
+                for k in range(j, o):
+                    r = bqc.bqc_t_triplet_owner(o, nshard, i, j, k)
+                    assert 0 <= r < nshard
+                    seen[(i, j, k)] = r
+        counts = [list(seen.values()).count(r) for r in range(nshard)]
+        assert sum(counts) == bqc.bqc_t_num_triplets(o) and max(counts) - min(counts) <= 1
+        total = sum(bqc.bqc_t_flops(o, 9, bqc.make_opts(shard_rank=r, shard_count=nshard)) for r in range(nshard))
+        assert total == bqc.bqc_t_flops(o, 9)
+    assert bqc.bqc_t_triplet_owner(o, 0, 0, 1, 2) == -1
+
+
+def test_plan_and_workspace(libpath):
+    import paper_2502_17963_b200 as bqc
+    assert bqc.bqc_t_plan_occ_block(5, 19, 84) == 5
+    bo5 = bqc.bqc_t_plan_occ_block(100, 380, 1680)
+    # config 5: the (vv|ov) tensor (43.9 GB) is never resident: 4*Bo slabs only
+    assert 1 <= bo5 <= 25
+    ws5 = bqc.bqc_t_workspace_bytes(100, 380, 1680)
+    assert 10e9 < ws5 < 150e9
+    assert bqc.bqc_t_workspace_bytes(100, 380, 1680, bqc.make_opts(occ_block=2)) < ws5
+    # invalid arguments are reported, not crashed on
+    assert bqc.bqc_t_workspace_bytes(0, 19, 84) == 0 and bqc.bqc_last_error() == 1
+    assert bqc.bqc_t_workspace_bytes(5, 19, 84, bqc.make_opts(occ_lo=3, occ_hi=2)) == 0
+    assert bqc.bqc_last_error() == 9
+    assert "option" in bqc.bqc_error_string(9)
+    assert bqc.bqc_error_string(0) == "ok"

@@ -1,0 +1,218 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerances: energies |dE| <= 1e-10 |E| + 1e-12 Eh (BASELINE.json north_star); intermediates
+(slabs, W, V) |d| <= 1e-11 * max|x| — FP64 sums of <= 6(v+o)+naux products in a different order
+than the oracle's BLAS.
+"""
+import numpy as np
+import pytest
+import torch
+
+import paper_2502_17963_b200 as bqc
+from bqc_inputs import make_config, make_inputs, sample_triplets, worked_example
+from gpu_util import dims, e_tol, to_device
+from oracle import t_oracle as orc
+
+pytestmark = pytest.mark.gpu
+
+
+def _close(got, ref, rel=1e-11):
+    got = got.cpu().numpy() if isinstance(got, torch.Tensor) else np.asarray(got)
+    scale = np.max(np.abs(ref)) + 1e-300
+    err = np.max(np.abs(got - ref))
+    assert err <= rel * scale, f"max err {err:.3e} vs scale {scale:.3e}"
+
+
+# ------------------------------------------------------------------ the tile-GEMM engine alone
+@pytest.mark.parametrize("M,N,K", [(128, 128, 16), (1, 1, 1), (130, 70, 37), (517, 261, 100), (64, 300, 480),
+                                   (1000, 19, 24)])
+def test_dgemm_nt(M, N, K):
+    rng = np.random.default_rng(M * 7 + N * 3 + K)
+    lda = K + (K % 2) + 2
+    A = np.zeros((M, lda)); A[:, :K] = rng.normal(size=(M, K))
+    B = np.zeros((N, lda)); B[:, :K] = rng.normal(size=(N, K))
+    A[:, K:] = 7.0   # stride padding must never be read as data
+    B[:, K:] = -3.0
+    dA = torch.from_numpy(A).cuda()[:, :K]
+    dB = torch.from_numpy(B).cuda()[:, :K]
+    C = bqc.bqc_dgemm_nt(dA, dB)
+    _close(C, A[:, :K] @ B[:, :K].T, rel=1e-13 * max(K, 16))
+
+
+# ------------------------------------------------------------------ row a1: DF slabs
+@pytest.mark.parametrize("case", ["config1", "odd", "config2"])
+def test_df_slabs(case):
+    inp = {"config1": lambda: make_config(1), "odd": lambda: make_inputs(3, 21, 13, seed=5),
+           "config2": lambda: make_config(2)}[case]()
+    d = to_device(inp)
+    o = inp.nocc
+    for (x, y) in [(0, 0), (o - 1, 1), (1, o - 1)]:
+        I, O, J = bqc.bqc_t_debug_slabs(*dims(inp), d[3], d[4], d[5], d[6], x, y)
+        _close(I, orc.slab_vvov(inp, x))
+        _close(O, orc.slab_ooov(inp, x, y))
+        _close(J, orc.slab_ovov(inp, x, y))
+
+
+# ------------------------------------------------------------------ rows a2 + a3: W and V
+@pytest.mark.parametrize("case", ["worked346", "config1", "ragged", "config2"])
+def test_w_and_v_elementwise(case):
+    inp = {"worked346": lambda: worked_example(3, 4, 6), "config1": lambda: make_config(1),
+           "ragged": lambda: make_inputs(4, 35, 41, seed=8, t1_std=0.05),
+           "config2": lambda: make_config(2, t1_std=0.05)}[case]()
+    d = to_device(inp)
+    o = inp.nocc
+    trips = [(0, 1, 2), (0, 0, o - 1), (1, o - 1, o - 1), (2, 0, 1), (1, 1, 1)]
+    if case == "config2":
+        trips = [(3, 11, 19), (7, 7, 2)]
+    for (i, j, k) in trips:
+        W, V = bqc.bqc_t_debug_wv(*dims(inp), *d, i, j, k)
+        Wr = orc.w_triplet(inp, i, j, k)
+        _close(W, Wr)
+        _close(V, orc.v_triplet(inp, i, j, k, Wr))
+
+
+# ------------------------------------------------------------------ rows a4 + a5: energies
+SMALL = {
+    "worked234": lambda: worked_example(2, 3, 4),
+    "worked346": lambda: worked_example(3, 4, 6),
+    "config1": lambda: make_config(1),
+    "config1_t1": lambda: make_config(1, t1_std=0.05),          # a3 exercised at O(1) weight
+    "v16": lambda: make_inputs(3, 16, 10, seed=31, t1_std=0.05),  # exactly one 16-block
+    "v17": lambda: make_inputs(4, 17, 9, seed=32, t1_std=0.05),   # ragged tail of 1
+    "v33": lambda: make_inputs(3, 33, 20, seed=33, t1_std=0.05),  # 3 blocks, ragged
+    "o2": lambda: make_inputs(2, 9, 5, seed=34, t1_std=0.05),
+}
+
+
+@pytest.mark.parametrize("case", sorted(SMALL))
+def test_energy_small_full(case):
+    inp = SMALL[case]()
+    d = to_device(inp)
+    e_ref, trip_ref = orc.t_energy(inp, return_triplets=True)
+    et = torch.empty(bqc.bqc_t_num_triplets(inp.nocc), dtype=torch.float64, device="cuda")
+    e = bqc.bqc_t_energy_ex(*dims(inp), *d, e_triplet=et)
+    assert abs(e - e_ref) <= e_tol(e_ref)
+    got = et.cpu().numpy()
+    n = len(trip_ref)
+    assert np.all(np.abs(got - trip_ref) <= 1e-10 * np.abs(trip_ref) + 1e-12 * abs(e_ref) / n + 1e-300)
+    # plain entry point
+    assert bqc.bqc_t_energy(*dims(inp), *d) == e
+
+
+def test_golden_worked_example_values():
+    # SURVEY.md §8(c) P2 (tests/golden/worked_examples.txt)
+    for shape, want in {(2, 3, 4): -9.406698159242249e-07, (3, 4, 6): -1.851157457841839e-04}.items():
+        inp = worked_example(*shape)
+        e = bqc.bqc_t_energy(*dims(inp), *to_device(inp))
+        assert abs(e - want) <= e_tol(want)
+
+
+def test_no_t1_flag_gives_e4():
+    inp = make_config(1, t1_std=0.05)
+    e4 = orc.t_energy(inp, with_t1=False)
+    e = bqc.bqc_t_energy_ex(*dims(inp), *to_device(inp), opts=bqc.make_opts(flags=bqc.BQC_T_FLAG_NO_T1))
+    assert abs(e - e4) <= e_tol(e4)
+
+
+def test_single_occupied_is_exactly_zero():
+    inp = make_inputs(1, 6, 8, seed=2, t1_std=0.05, t2_std=0.05)
+    assert bqc.bqc_t_energy(*dims(inp), *to_device(inp)) == 0.0
+
+
+@pytest.mark.parametrize("cfg,count", [(2, 10), (3, 5)])
+def test_energy_sampled_triplets(cfg, count):
+    inp = make_config(cfg)
+    d = to_device(inp)
+    o = inp.nocc
+    et = torch.empty(bqc.bqc_t_num_triplets(o), dtype=torch.float64, device="cuda")
+    e = bqc.bqc_t_energy_ex(*dims(inp), *d, e_triplet=et)
+    got = et.cpu().numpy()
+    assert abs(got.sum() - e) <= 1e-12 * abs(e)
+    n = len(got)
+    for (i, j, k) in sample_triplets(o, count, seed=100 + cfg):
+        ref = orc.e_triplet(inp, i, j, k)
+        g = got[bqc.bqc_t_triplet_index(o, i, j, k)]
+        assert abs(g - ref) <= 1e-10 * abs(ref) + 1e-12 * abs(e) / n, (i, j, k, g, ref)
+    # properties that hold at any size: diagonal triplets are exactly 0, E[4]-dominated values < 0
+    for i in range(o):
+        assert got[bqc.bqc_t_triplet_index(o, i, i, i)] == 0.0
+    assert np.all(got <= 0.0)
+
+
+# ------------------------------------------------------------------ scheduler: windows, blocks, shards
+def test_blocking_window_and_sharding_agree_bitwise():
+    inp = make_inputs(7, 20, 18, seed=41, t1_std=0.02)
+    d = to_device(inp)
+    n = bqc.bqc_t_num_triplets(7)
+    base = torch.empty(n, dtype=torch.float64, device="cuda")
+    e = bqc.bqc_t_energy_ex(*dims(inp), *d, e_triplet=base)
+    assert abs(e - orc.t_energy(inp)) <= e_tol(e)
+    for bo, mb in [(1, 1), (2, 3), (3, 0), (4, 2)]:
+        et = torch.empty_like(base)
+        e2 = bqc.bqc_t_energy_ex(*dims(inp), *d, opts=bqc.make_opts(occ_block=bo, max_batch=mb), e_triplet=et)
+        assert torch.equal(et, base), (bo, mb)     # same per-triplet arithmetic whatever the blocking
+        assert e2 == e
+    # shards: disjoint supports that add up to the whole
+    parts = []
+    for r in range(3):
+        et = torch.empty_like(base)
+        bqc.bqc_t_energy_ex(*dims(inp), *d, opts=bqc.make_opts(shard_rank=r, shard_count=3, occ_block=3), e_triplet=et)
+        parts.append(et)
+    assert torch.equal(parts[0] + parts[1] + parts[2], base)
+    for idx in range(n):
+        assert sum(int(p[idx] != 0) for p in parts) <= 1
+    # window: only triplets inside [2,6)
+    et = torch.empty_like(base)
+    ew = bqc.bqc_t_energy_ex(*dims(inp), *d, opts=bqc.make_opts(occ_lo=2, occ_hi=6), e_triplet=et)
+    ref = 0.0
+    for (i, j, k) in orc.triplet_list(7):
+        idx = bqc.bqc_t_triplet_index(7, i, j, k)
+        if 2 <= i and k < 6:
+            assert et[idx] == base[idx]
+            ref += orc.e_triplet(inp, i, j, k)
+        else:
+            assert et[idx] == 0.0
+    assert abs(ew - ref) <= e_tol(ref)
+
+
+def test_deterministic_and_workspace_and_host_paths():
+    inp = make_config(1, t1_std=0.01)
+    d = to_device(inp)
+    e1 = bqc.bqc_t_energy(*dims(inp), *d)
+    e2 = bqc.bqc_t_energy(*dims(inp), *d)
+    assert e1 == e2                                             # bit-identical
+    ws = torch.empty(bqc.bqc_t_workspace_bytes(*dims(inp)), dtype=torch.uint8, device="cuda")
+    assert bqc.bqc_t_energy_ex(*dims(inp), *d, workspace=ws) == e1
+    with pytest.raises(bqc.BqcError) as ei:
+        bqc.bqc_t_energy_ex(*dims(inp), *d, workspace=ws[:1024])
+    assert ei.value.code == 5
+    host = [torch.from_numpy(a) for a in inp.arrays()]
+    eh, h2d, d2h = bqc.bqc_t_energy_host(*dims(inp), *host)
+    assert eh == e1 and h2d == inp.nbytes() and d2h == 8
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        assert bqc.bqc_t_energy(*dims(inp), *d) == e1           # non-default stream
+
+
+# ------------------------------------------------------------------ error behaviour (no CPU fallback)
+def test_errors_are_reported():
+    inp = make_config(1)
+    d = to_device(inp)
+    o, v, x = dims(inp)
+    L = bqc.lib()
+    import ctypes
+    ptrs = [ctypes.c_void_p(t.data_ptr()) for t in d]
+    e = ctypes.c_double(0)
+    def call(o_=o, v_=v, x_=x, p=ptrs):
+        return L.bqc_t_energy_ex(o_, v_, x_, *p, None, None, 0, ctypes.byref(e), None, None)
+    assert call(o_=0) == 1
+    assert call(p=[None] + ptrs[1:]) == 2
+    host = torch.from_numpy(inp.t2)
+    assert call(p=ptrs[:3] + [ctypes.c_void_p(host.data_ptr())] + ptrs[4:]) == 3
+    assert call(p=[ctypes.c_void_p(d[0].data_ptr() + 4)] + ptrs[1:]) == 4
+    bad = d[0].clone(); bad[-1] = 1.0                            # occupied level above a virtual one
+    assert call(p=[ctypes.c_void_p(bad.data_ptr())] + ptrs[1:]) == 8
+    assert L.bqc_last_error() == 8 and b"denominator" in L.bqc_error_detail()
+    import math
+    assert math.isnan(L.bqc_t_energy(0, v, x, *ptrs, None))
+    assert call() == 0                                           # and the library still works
