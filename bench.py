@@ -1,0 +1,321 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the B200-native closed-shell (T) energy path.
+
+    python bench.py --gpus N --steps K --warmup W [--config 5] [--window 10] [--full]
+    python bench.py --impl reference ...        # the CPU oracle on the same workload (bounded sample)
+
+A "step" is one pass of the whole hot path (DF slab former -> W builder -> fused V -> energy
+contraction -> fixed-order sums) over one batch of occupied-triplet
+blocks of the workload.  Default workload: BASELINE.json configs[4] (nocc=100 nvir=380 naux=1680,
+the configuration the >= 60 % target is quoted on), one triplet block per GPU = all triplets
+i<=j<=k inside an occupied window of `--window` orbitals (rank r takes window [r*w, (r+1)*w)):
+weak scaling, no data-path collective (triplets are independent; the only exchange is one scalar
+sum).  `--full` evaluates the complete E(T) of the config in one step instead.
+
+value = algorithmic W-builder FP64 flops of the step (bqc_t_flops: #triplets * 12 v^3 (v+o); slab
+forming and the energy contraction are NOT credited) / max-over-ranks device time, in TFLOP/s.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+METRIC = "(T) FP64 TFLOP/s (W-builder algorithmic flops / whole-path time)"
+UNIT = "TFLOP/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json configs[n-1], n = 1..5")
+    ap.add_argument("--window", type=int, default=10, help="occupied orbitals per triplet block (per GPU)")
+    ap.add_argument("--full", action="store_true", help="whole E(T) of the config in one step")
+    ap.add_argument("--occ-block", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=1)
+    ap.add_argument("--peak-seconds", type=float, default=2.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(cfg, c, lo, hi, full, ntrip):
+    base = f"config{cfg} nocc={c['nocc']} nvir={c['nvir']} naux={c['naux']} (synthetic water-cluster shape)"
+    if full:
+        return base + f", full E(T): all {ntrip} triplets i<=j<=k"
+    return base + f", one triplet block per GPU: occupied window [{lo},{hi}) = {ntrip} triplets"
+
+
+# ----------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu = gpu_index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.gpu)],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()        # the exact PID we started
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); smax.append(float(f[2])); power.append(float(f[3]))
+            except ValueError:
+                continue
+            for n, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "power_w_max": float(max(power)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------- reference arm (oracle)
+def oracle_sample(inp, triplet):
+    """Time the oracle as it stands on one triplet of the workload; returns (seconds, e_ijk)."""
+    from oracle import t_oracle as orc      # bench.py's cpu_baseline / --impl reference leg only
+    t0 = time.perf_counter()
+    e = orc.e_triplet(inp, *triplet)
+    return time.perf_counter() - t0, e
+
+
+def cpu_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = max((p.get("num_threads", 1) for p in threadpool_info()), default=1)
+        return int(n)
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    from bqc_inputs import CONFIGS, make_config
+    c = CONFIGS[args.config]
+    o, v = c["nocc"], c["nvir"]
+    inp = make_config(args.config)
+    lo, hi = (0, o) if args.full else (0, min(args.window, o))
+    trip = (lo, (lo + hi - 1) // 2, hi - 1)
+    flops = 12.0 * v ** 3 * (v + o)
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(inp, trip)
+    times = []
+    for _ in range(args.steps):
+        dt, _e = oracle_sample(inp, trip)
+        times.append(dt)
+    dt = float(np.mean(times))
+    val = flops / dt * 1e-12
+    ntrip = (hi - lo) * (hi - lo + 1) * (hi - lo + 2) // 6
+    sample = f"one triplet {trip} of the workload per step (12 v^3 (v+o) = {flops:.3e} flops), NumPy/OpenBLAS oracle"
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": workload_name(args.config, c, lo, hi, args.full, ntrip), "sample": sample},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle", "sample": sample},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+# ----------------------------------------------------------------------------- our arm
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch.distributed as dist
+    import paper_2502_17963_b200 as bqc
+    from bqc_inputs import CONFIGS, make_config
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the CUDA library is the only implementation")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    c = CONFIGS[args.config]
+    o, v, X = c["nocc"], c["nvir"], c["naux"]
+    w = o if args.full else min(args.window, o)
+    nblocks = max(1, o // w)
+    lo = 0 if args.full else (rank % nblocks) * w
+    hi = o if args.full else lo + w
+    if args.full and world > 1:
+        opts = bqc.make_opts(occ_block=args.occ_block, shard_rank=rank, shard_count=world,
+                             flags=bqc.BQC_T_FLAG_PROFILE)
+    else:
+        opts = bqc.make_opts(occ_block=args.occ_block, occ_lo=lo, occ_hi=hi, flags=bqc.BQC_T_FLAG_PROFILE)
+    flops_rank = bqc.bqc_t_flops(o, v, opts)
+    ntrip = int(round(flops_rank / (12.0 * v ** 3 * (v + o))))
+
+    t0 = time.perf_counter()
+    inp = make_config(args.config)
+    gen_s = time.perf_counter() - t0
+    host = [torch.from_numpy(a) for a in inp.arrays()]
+    try:
+        host = [t.pin_memory() for t in host]          # e2e copies come from pinned memory
+        pinned = True
+    except RuntimeError:
+        pinned = False
+    dev = [t.cuda(non_blocking=True) for t in host]
+    torch.cuda.synchronize()
+    ws = torch.empty(bqc.bqc_t_workspace_bytes(o, v, X, opts), dtype=torch.uint8, device="cuda")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # FP64 tensor-core peak measured in this run: the roofline denominator
+    peak_dmma = bqc.bqc_fp64_peak_tflops(0, args.peak_seconds)
+
+    def step():
+        return bqc.bqc_t_energy_ex(o, v, X, *dev, opts=opts, workspace=ws)
+
+    for _ in range(args.warmup):
+        e_val = step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches = 0
+    prof = None
+    ev0.record()
+    for _ in range(args.steps):
+        e_val = step()
+        prof = bqc.bqc_t_last_profile()
+        launches += int(prof["kernel_launches"])
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1) / max(args.steps, 1)
+    peak_after = bqc.bqc_fp64_peak_tflops(0, min(args.peak_seconds, 1.0))
+    peak = max(peak_dmma, peak_after)
+
+    # end to end through the C ABI with HOST buffers (H2D of all inputs + D2H of the scalar inside)
+    e2e_ms, h2d, d2h = None, 0, 0
+    if args.e2e_steps > 0:
+        del ws
+        torch.cuda.empty_cache()
+        eopts = bqc.make_opts(occ_block=args.occ_block, occ_lo=opts.occ_lo, occ_hi=opts.occ_hi,
+                              shard_rank=opts.shard_rank, shard_count=opts.shard_count)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            e_host, h2d, d2h = bqc.bqc_t_energy_host(o, v, X, *host, opts=eopts)
+        torch.cuda.synchronize()
+        e2e_ms = (time.perf_counter() - t0) * 1e3 / args.e2e_steps
+        assert e_host == e_val, "e2e result differs from the device-resident result"
+
+    # max over ranks, whole-job aggregate
+    t = torch.tensor([ms, e2e_ms or 0.0, float(flops_rank)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        tmax = t.clone()
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone()
+        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        ms, e2e_ms_max, flops_total = float(tmax[0]), float(tmax[1]), float(tsum[2])
+        esum = torch.tensor([e_val], dtype=torch.float64, device="cuda")
+        dist.all_reduce(esum, op=dist.ReduceOp.SUM)        # the path's one exchange: a scalar
+        e_total = float(esum[0])
+    else:
+        e2e_ms_max, flops_total, e_total = (e2e_ms or 0.0), float(flops_rank), e_val
+
+    if rank == 0:
+        value = flops_total / (ms * 1e-3) * 1e-12
+        flops_full = bqc.bqc_t_flops(o, v)
+        gemm_tf = flops_rank / (prof["gemm_ms"] * 1e-3) * 1e-12 if prof["gemm_ms"] > 0 else None
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config, c, lo, hi, args.full, ntrip),
+                       "triplets_per_gpu": ntrip, "occ_block": bqc.bqc_t_plan_occ_block(o, v, X, opts),
+                       "l2": "inputs larger than L2 (554 MB augmented slabs, 1.4 GB F per triplet); no flush needed"
+                             if args.config >= 4 else "working set may fit L2 on small configs",
+                       "timing": "CUDA events on the launch stream around K bqc_t_energy_ex calls, max over ranks",
+                       "pinned_host": pinned, "input_gen_s": round(gen_s, 1)},
+            "pct_of_fp64_tensor_peak": 100.0 * value / (peak * world),
+            "fp64_tensor_peak_tflops_measured": peak,
+            "seconds_per_step": ms * 1e-3,
+            "seconds_per_full_E_T_extrapolated": flops_full / (value * 1e12),
+            "e_t_of_step_hartree": e_total,
+            "kernel_ms_per_step": {"w_builder": prof["gemm_ms"], "energy": prof["energy_ms"],
+                                   "slab_former": prof["form_ms"], "prepare": prof["prepare_ms"],
+                                   "call_total": prof["total_ms"]},
+            "roofline": {"bound": "tensor", "kernel": "gemm_nt_kernel (W builder, row a2)",
+                         "achieved": gemm_tf, "peak": peak, "unit": UNIT,
+                         "frac": (gemm_tf / peak) if gemm_tf else None,
+                         "peak_source": "FP64 DMMA peak measured in this run by bqc_fp64_peak_tflops (register-resident "
+                                        "mma.sync m8n8k4 loop on all SMs); MEASURED_PEAKS.json has no FP64 entry",
+                         "launches": int(prof["gemm_launches"]),
+                         "flops_per_launch": flops_rank / max(prof["gemm_launches"], 1),
+                         "traffic": None},
+            "clocks": clocks,
+            "e2e": {"value": (flops_total / (e2e_ms_max * 1e-3) * 1e-12) if e2e_ms_max else None, "unit": UNIT,
+                    "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "ms_per_step": e2e_ms_max, "steps": args.e2e_steps},
+            "gpu_launches": launches,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            trip = (lo, (lo + hi - 1) // 2, hi - 1)
+            dt, e_ref = oracle_sample(inp, trip)
+            f1 = 12.0 * v ** 3 * (v + o)
+            out["cpu_baseline"] = {"value": f1 / dt * 1e-12, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
+                                   "sample": f"one triplet {trip} of the workload ({f1:.3e} flops) in {dt:.1f} s, "
+                                             "NumPy/OpenBLAS oracle as it stands"}
+        print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -70,7 +70,9 @@ typedef struct bqc_t_opts {
 } bqc_t_opts;
 
 enum {
-  BQC_T_FLAG_NO_T1 = 1          /* drop the t1 (E[5]) term: V = W (for the E[4]-only checks)  */
+  BQC_T_FLAG_NO_T1 = 1,         /* drop the t1 (E[5]) term: V = W (for the E[4]-only checks)  */
+  BQC_T_FLAG_PROFILE = 2        /* bracket every kernel group with CUDA events on its launching
+                                   stream; read the sums with bqc_t_last_profile             */
 };
 
 /* ---- host-only helpers (no GPU needed) -------------------------------------------------- */
@@ -122,6 +124,16 @@ BQC_API int bqc_t_energy_ex(int nocc, int nvir, int naux,
                     const double* B_oo, const double* B_ov, const double* B_vv,
                     const bqc_t_opts* opts, void* workspace, size_t workspace_bytes,
                     double* e_total_host, double* e_triplet_dev, void* stream);
+
+/* Timing of the last bqc_t_energy_ex call of this thread that had BQC_T_FLAG_PROFILE set, measured
+   with CUDA events on the streams the kernels were launched on.  Fills up to n (<= 9) doubles:
+     [0] W-builder (tile-GEMM) kernel milliseconds, summed over launches   [1] number of those launches
+     [2] energy-contraction + per-triplet reduction kernel milliseconds     [3] number of those launches
+     [4] slab-former milliseconds (DF GEMM + hole columns, former stream)   [5] number of slab blocks formed
+     [6] input repacking + B~/J formation milliseconds                      [7] whole call, first to last kernel
+     [8] number of library kernels launched by the call (counted whether or not PROFILE was set)
+   Returns the number of values written (n <= 9). */
+BQC_API int bqc_t_last_profile(double* out, int n);
 
 /* End-to-end form: every array argument is a HOST pointer (pinned or pageable).  Inputs are
    copied to the device, E(T) is evaluated by the same kernels, the scalar (and, if

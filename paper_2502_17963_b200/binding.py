@@ -30,6 +30,7 @@ class bqc_t_opts(Structure):
 
 
 BQC_T_FLAG_NO_T1 = 1
+BQC_T_FLAG_PROFILE = 2
 
 _lib = None
 
@@ -66,6 +67,8 @@ def lib():
     L.bqc_t_energy_ex.restype = c_int
     L.bqc_t_energy_ex.argtypes = [c_int] * 3 + [dp] * 7 + [POINTER(bqc_t_opts), c_void_p, c_size_t,
                                                          POINTER(c_double), dp, c_void_p]
+    L.bqc_t_last_profile.restype = c_int
+    L.bqc_t_last_profile.argtypes = [POINTER(c_double), c_int]
     L.bqc_t_energy_host.restype = c_int
     L.bqc_t_energy_host.argtypes = [c_int] * 3 + [dp] * 7 + [POINTER(bqc_t_opts), POINTER(c_double), dp,
                                                            POINTER(c_size_t), POINTER(c_size_t), c_void_p]
@@ -191,6 +194,15 @@ def bqc_t_energy_ex(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv
     _check(lib().bqc_t_energy_ex(nocc, nvir, naux, *p, _optp(opts), ws_ptr, ws_bytes, byref(e), et,
                                  _stream()))
     return e.value
+
+
+def bqc_t_last_profile():
+    """Kernel-group timings of the last profiled bqc_t_energy_ex call (see include/bqc_t.h)."""
+    buf = (c_double * 9)()
+    n = lib().bqc_t_last_profile(buf, 9)
+    keys = ["gemm_ms", "gemm_launches", "energy_ms", "energy_launches", "form_ms", "form_blocks",
+            "prepare_ms", "total_ms", "kernel_launches"]
+    return {k: buf[i] for i, k in enumerate(keys[:n])}
 
 
 def bqc_t_energy_host(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, opts=None,

@@ -14,6 +14,8 @@ namespace bqc {
 // ------------------------------------------------------------------ error state (thread-local)
 void set_error(int code, const char* fmt, ...);
 void clear_error();
+// number of kernels this thread launched (every launch_* helper counts its kernels)
+void count_launch(int n = 1);
 
 #define BQC_CUDA_OK(expr)                                                                   \
   do {                                                                                      \

@@ -202,6 +202,7 @@ int launch_energy(const EnergyArgs& a, cudaStream_t s) {
   if (a.ntrip <= 0) return BQC_OK;
   dim3 grid(a.norbits, a.ntrip);
   energy_kernel<<<grid, kEThreads, sizeof(EnergySmem), s>>>(a);
+  count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
 }
@@ -232,6 +233,7 @@ int launch_reduce_triplets(const double* partial, const TripletRec* trips, int n
                            double* e_trip, cudaStream_t s) {
   if (ntrip <= 0) return BQC_OK;
   reduce_triplets_kernel<<<ntrip, 256, 0, s>>>(partial, trips, norbits, e_trip);
+  count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
 }
@@ -251,6 +253,7 @@ __global__ void final_sum_kernel(const double* __restrict__ e, long long n, doub
 
 int launch_final_sum(const double* e_trip, long long n, double* out, cudaStream_t s) {
   final_sum_kernel<<<1, 1024, 0, s>>>(e_trip, n, out);
+  count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
 }
@@ -286,6 +289,7 @@ int launch_assemble_wv(const double* F, int nb16, int v, const double* J, int nw
   assemble_wv_kernel<<<1024, 256, 0, s>>>(F, nb16, v, J + ((size_t)pj * nw + pk) * v2,
                                           J + ((size_t)pi * nw + pk) * v2, J + ((size_t)pi * nw + pj) * v2,
                                           t1i, t1j, t1k, W, V);
+  count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
 }

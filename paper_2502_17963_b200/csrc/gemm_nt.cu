@@ -89,6 +89,7 @@ static int launch_nf(const CUtensorMap& tmA, const CUtensorMap& tmAT, const CUte
   });
   BQC_CUDA_OK(attr_err);
   gemm_nt_kernel<NF><<<grid, kGemmThreads, gemm_smem_bytes(NF), stream>>>(tmA, tmAT, tmB, prm);
+  count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
 }

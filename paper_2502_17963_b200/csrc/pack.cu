@@ -23,6 +23,7 @@ __global__ void transpose_pad_kernel(const double* __restrict__ in, double* __re
 int launch_transpose_pad(const double* in, double* out, int nq, int nr, int qp, cudaStream_t s) {
   dim3 grid(ceil_div(nr, 32), ceil_div(qp, 32));
   transpose_pad_kernel<<<grid, dim3(32, 8), 0, s>>>(in, out, nq, nr, qp);
+  count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
 }
@@ -44,6 +45,7 @@ int launch_btilde_t2(const double* t2, double* btil, int o, int v, const int* ac
                      cudaStream_t s) {
   const long long rows = (long long)na * na * v;
   btilde_t2_kernel<<<(unsigned)rows, 128, 0, s>>>(t2, btil, o, v, act_dev, na, kp);
+  count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
 }
@@ -78,6 +80,7 @@ int launch_slab_holes(const double* t2, double* slabs, int o, int v, int kp, int
   const size_t v2 = (size_t)v * v;
   dim3 grid((unsigned)((v2 + 31) / 32), ceil_div(o, 32), nx);
   slab_holes_kernel<<<grid, dim3(32, 8), 0, s>>>(t2, slabs, o, v, kp, x0, slot0);
+  count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
 }
@@ -102,6 +105,7 @@ int launch_copy3(const double* in, long long sa, long long sb, long long sc, dou
   if (total <= 0) return BQC_OK;
   const int grid = (int)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
   copy3_kernel<<<grid, 256, 0, s>>>(in, sa, sb, sc, out, na, nb, nc);
+  count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
 }

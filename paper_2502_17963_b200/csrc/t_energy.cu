@@ -37,6 +37,10 @@ void clear_error() {
   g_detail[0] = 0;
 }
 
+static thread_local double g_profile[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+static thread_local long long g_launches = 0;
+void count_launch(int n) { g_launches += n; }
+
 namespace {
 
 // ------------------------------------------------------------------ plan
@@ -52,6 +56,7 @@ struct Plan {
   int nbatch = 0;              // triplets per W-builder launch
   int norbits = 0;
   int use_t1 = 1;
+  int profile = 0;
   int shard_rank = 0, shard_count = 1;
   // workspace offsets (bytes)
   size_t off_btvv = 0, off_btov = 0, off_btoo = 0, off_btil = 0, off_J = 0, off_slabs = 0, off_F = 0,
@@ -108,6 +113,7 @@ int make_plan(Plan& P, int o, int v, int X, const std::vector<int>& act, const b
   P.slab_elems = (size_t)v * v * P.Kp;
   P.norbits = P.nb16 * (P.nb16 + 1) * (P.nb16 + 2) / 6;
   P.use_t1 = !(opts && (opts->flags & BQC_T_FLAG_NO_T1));
+  P.profile = (opts && (opts->flags & BQC_T_FLAG_PROFILE)) ? 1 : 0;
   P.shard_count = (opts && opts->shard_count > 0) ? opts->shard_count : 1;
   P.shard_rank = opts ? opts->shard_rank : 0;
   if (P.shard_rank < 0 || P.shard_rank >= P.shard_count) {
@@ -227,6 +233,17 @@ struct Ctx {
   // host schedule
   std::vector<GemmTask> tasks;
   std::vector<TripletRec> trips;
+  // BQC_T_FLAG_PROFILE: timing events, [3n] before W builder, [3n+1] after it, [3n+2] after the energy kernels
+  std::vector<cudaEvent_t> prof_main;
+  std::vector<cudaEvent_t> prof_form;   // [2n], [2n+1] around each slab-block formation
+  cudaEvent_t prof_begin = nullptr, prof_prepared = nullptr, prof_end = nullptr;
+  int prof_mark(std::vector<cudaEvent_t>& v, cudaStream_t s) {
+    cudaEvent_t e;
+    BQC_CUDA_OK(cudaEventCreate(&e));
+    v.push_back(e);
+    BQC_CUDA_OK(cudaEventRecord(e, s));
+    return BQC_OK;
+  }
 
   double* d(size_t off) const { return reinterpret_cast<double*>(ws + off); }
   double* btvv() const { return d(P.off_btvv); }
@@ -245,6 +262,11 @@ struct Ctx {
   TripletRec* trips_dev() const { return reinterpret_cast<TripletRec*>(ws + P.off_trips); }
 
   ~Ctx() {
+    for (cudaEvent_t e : prof_main) cudaEventDestroy(e);
+    for (cudaEvent_t e : prof_form) cudaEventDestroy(e);
+    if (prof_begin) cudaEventDestroy(prof_begin);
+    if (prof_prepared) cudaEventDestroy(prof_prepared);
+    if (prof_end) cudaEventDestroy(prof_end);
     for (int s = 0; s < 4; ++s) {
       if (ev_formed[s]) cudaEventDestroy(ev_formed[s]);
       if (ev_free[s]) cudaEventDestroy(ev_free[s]);
@@ -599,7 +621,9 @@ int Pipeline::compute(const Action& a) {
   prm.n2_ext = 1;
   prm.tasks = c.tasks_dev() + a.task0;
   prm.C = c.F();
+  if (P.profile) BQC_TRY(c.prof_mark(c.prof_main, s));
   BQC_TRY(launch_gemm_nt(c.f_nf, c.tm_slab, c.tm_slabT, c.tm_btil, prm, s));
+  if (P.profile) BQC_TRY(c.prof_mark(c.prof_main, s));
 
   EnergyArgs e;
   e.F = c.F(); e.trips = c.trips_dev() + a.trip0; e.orbits = c.orbits_dev();
@@ -608,6 +632,7 @@ int Pipeline::compute(const Action& a) {
   e.ntrip = (int)a.ntrip; e.norbits = P.norbits; e.nb16 = P.nb16; e.v = v; e.nw = P.na; e.use_t1 = P.use_t1;
   BQC_TRY(launch_energy(e, s));
   BQC_TRY(launch_reduce_triplets(c.partial(), c.trips_dev() + a.trip0, (int)a.ntrip, P.norbits, c.etrip(), s));
+  if (P.profile) BQC_TRY(c.prof_mark(c.prof_main, s));
   return BQC_OK;
 }
 
@@ -616,7 +641,9 @@ int Pipeline::execute() {
     if (a.kind == Action::FORM) {
       // the former stream may overwrite a slot set only after the main stream's last use of it
       if (c.ev_free_valid[a.set]) BQC_CUDA_OK(cudaStreamWaitEvent(c.s_form, c.ev_free[a.set], 0));
+      if (c.P.profile) BQC_TRY(c.prof_mark(c.prof_form, c.s_form));
       BQC_TRY(form_block(a.set, a.block, c.s_form));
+      if (c.P.profile) BQC_TRY(c.prof_mark(c.prof_form, c.s_form));
       BQC_CUDA_OK(cudaEventRecord(c.ev_formed[a.set], c.s_form));
       BQC_CUDA_OK(cudaStreamWaitEvent(c.s_main, c.ev_formed[a.set], 0));
     } else {
@@ -686,16 +713,51 @@ int t_energy_impl(int o, int v, int X, const Inputs& in, const bqc_t_opts* opts,
 
   Pipeline p;
   BQC_TRY(p.setup(o, v, X, in, act, opts, workspace, workspace_bytes, stream));
+  Ctx& c = p.c;
+  const bool prof = c.P.profile != 0;
+  const long long launches0 = g_launches;
+  if (prof) {
+    BQC_CUDA_OK(cudaEventCreate(&c.prof_begin));
+    BQC_CUDA_OK(cudaEventCreate(&c.prof_prepared));
+    BQC_CUDA_OK(cudaEventCreate(&c.prof_end));
+    BQC_CUDA_OK(cudaEventRecord(c.prof_begin, stream));
+  }
   BQC_TRY(p.build_schedule());
   BQC_TRY(p.prepare());
+  if (prof) BQC_CUDA_OK(cudaEventRecord(c.prof_prepared, stream));
   BQC_TRY(p.execute());
-  Ctx& c = p.c;
   BQC_TRY(launch_final_sum(c.etrip(), (long long)num_triplets(o), c.esum(), stream));
+  if (prof) BQC_CUDA_OK(cudaEventRecord(c.prof_end, stream));
   if (e_triplet_dev)
     BQC_CUDA_OK(cudaMemcpyAsync(e_triplet_dev, c.etrip(), num_triplets(o) * 8, cudaMemcpyDeviceToDevice, stream));
   BQC_CUDA_OK(cudaMemcpyAsync(e_total_host, c.esum(), 8, cudaMemcpyDeviceToHost, stream));
   BQC_CUDA_OK(cudaStreamSynchronize(stream));
   BQC_CUDA_OK(cudaStreamSynchronize(c.s_form));
+  g_profile[8] = (double)(g_launches - launches0);
+  if (prof) {
+    double gemm_ms = 0, en_ms = 0, form_ms = 0;
+    float ms = 0.f;
+    for (size_t n = 0; n + 2 < c.prof_main.size() + 1; n += 3) {
+      BQC_CUDA_OK(cudaEventElapsedTime(&ms, c.prof_main[n], c.prof_main[n + 1]));
+      gemm_ms += ms;
+      BQC_CUDA_OK(cudaEventElapsedTime(&ms, c.prof_main[n + 1], c.prof_main[n + 2]));
+      en_ms += ms;
+    }
+    for (size_t n = 0; n + 1 < c.prof_form.size(); n += 2) {
+      BQC_CUDA_OK(cudaEventElapsedTime(&ms, c.prof_form[n], c.prof_form[n + 1]));
+      form_ms += ms;
+    }
+    g_profile[0] = gemm_ms;
+    g_profile[1] = (double)(c.prof_main.size() / 3);
+    g_profile[2] = en_ms;
+    g_profile[3] = (double)(c.prof_main.size() / 3);
+    g_profile[4] = form_ms;
+    g_profile[5] = (double)(c.prof_form.size() / 2);
+    BQC_CUDA_OK(cudaEventElapsedTime(&ms, c.prof_begin, c.prof_prepared));
+    g_profile[6] = ms;
+    BQC_CUDA_OK(cudaEventElapsedTime(&ms, c.prof_begin, c.prof_end));
+    g_profile[7] = ms;
+  }
   return BQC_OK;
 }
 
@@ -760,6 +822,13 @@ size_t bqc_t_workspace_bytes(int nocc, int nvir, int naux, const bqc_t_opts* opt
   for (int x = lo; x < hi; ++x) act[x - lo] = x;
   if (make_plan(P, nocc, nvir, naux, act, opts) != BQC_OK) return 0;
   return P.total;
+}
+
+int bqc_t_last_profile(double* out, int n) {
+  if (!out || n <= 0) return 0;
+  const int m = n < 9 ? n : 9;
+  for (int i = 0; i < m; ++i) out[i] = g_profile[i];
+  return m;
 }
 
 int bqc_last_error(void) { return g_err; }
