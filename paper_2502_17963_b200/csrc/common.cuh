@@ -99,9 +99,12 @@ __device__ __forceinline__ void dmma_884(double& c0, double& c1, double a, doubl
                : "d"(a), "d"(b));
 }
 
+// ld.shared with a 32-bit shared-window address and a compile-time byte offset (folded into the
+// instruction's immediate field): no generic-address arithmetic in the GEMM inner loop.
+template <int OFF>
 __device__ __forceinline__ double lds_f64(uint32_t addr) {
   double v;
-  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+  asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(addr), "n"(OFF));
   return v;
 }
 

@@ -153,8 +153,23 @@ gemm_nt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   uint32_t koff[4];
 #pragma unroll
   for (int c = 0; c < 4; ++c) koff[c] = (uint32_t)((((c + 4 * (t >> 1)) ^ g) << 4) + ((t & 1) << 3));
-  const uint32_t a_row_off = (uint32_t)((warp_m0 + g) * (kBK * 8));
-  const uint32_t b_row_off = (uint32_t)(kBM * kBK * 8 + (warp_n0 + g) * (kBK * 8));
+  const uint32_t smem_base = smem_u32(smem);
+  const uint32_t a_base = smem_base + (uint32_t)((warp_m0 + g) * (kBK * 8));
+  const uint32_t b_base = smem_base + (uint32_t)(kBM * kBK * 8 + (warp_n0 + g) * (kBK * 8));
+
+  // fragments of one k4 step: 4 A values (rows g + 8i) and NF B values (rows g + 8j), plain ld.shared
+  auto load_frags = [&](double (&a)[4], double (&b)[NF], int stg, int c) {
+    const uint32_t off = (uint32_t)(stg * kStageBytes) + koff[c];
+    const uint32_t pa = a_base + off, pb = b_base + off;
+    a[0] = lds_f64<0 * 1024>(pa); a[1] = lds_f64<1 * 1024>(pa);
+    a[2] = lds_f64<2 * 1024>(pa); a[3] = lds_f64<3 * 1024>(pa);
+    b[0] = lds_f64<0 * 1024>(pb); b[1] = lds_f64<1 * 1024>(pb);
+    b[2] = lds_f64<2 * 1024>(pb); b[3] = lds_f64<3 * 1024>(pb);
+    if (NF > 4) b[4] = lds_f64<4 * 1024>(pb);
+    if (NF > 5) b[5 % NF] = lds_f64<5 * 1024>(pb);
+    if (NF > 6) b[6 % NF] = lds_f64<6 * 1024>(pb);
+    if (NF > 7) b[7 % NF] = lds_f64<7 * 1024>(pb);
+  };
 
   int stage = 0;
   uint32_t phase = 0;
@@ -173,26 +188,35 @@ gemm_nt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 #pragma unroll
       for (int j = 0; j < NF; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
+    // Fragments are double-buffered in registers across k4 steps AND across pipeline stages: the loads
+    // of step s+1 (possibly the first step of the next stage, after its full barrier) are issued before
+    // the 4*NF DMMAs of step s, so ld.shared latency and the barrier poll hide behind tensor work.
+    double fa[2][4], fb[2][NF];
+    mbar_wait(&full_bar[stage], phase);
+    load_frags(fa[0], fb[0], stage, 0);
     for (int it = 0; it < iters; ++it) {
-      mbar_wait(&full_bar[stage], phase);
-      const uint8_t* sbase = smem + stage * kStageBytes;
-      const uint8_t* pa = sbase + a_row_off;
-      const uint8_t* pb = sbase + b_row_off;
+      int nstage = stage + 1;
+      uint32_t nphase = phase;
+      if (nstage == kStages) { nstage = 0; nphase ^= 1u; }
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
-        double a[4], b[NF];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) a[i] = *reinterpret_cast<const double*>(pa + i * (8 * kBK * 8) + koff[c]);
-#pragma unroll
-        for (int j = 0; j < NF; ++j) b[j] = *reinterpret_cast<const double*>(pb + j * (8 * kBK * 8) + koff[c]);
+        const int cur = c & 1, nxt = cur ^ 1;
+        if (c < 3) {
+          load_frags(fa[nxt], fb[nxt], stage, c + 1);
+        } else if (it + 1 < iters) {
+          mbar_wait(&full_bar[nstage], nphase);
+          load_frags(fa[nxt], fb[nxt], nstage, 0);
+        }
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
-          for (int j = 0; j < NF; ++j) dmma_884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+          for (int j = 0; j < NF; ++j) dmma_884(acc[i][j][0], acc[i][j][1], fa[cur][i], fb[cur][j]);
       }
+      // every ld.shared of this stage was issued (and its value consumed by a DMMA above) -> release it
       __syncwarp();
       if (lane == 0) mbar_arrive(&empty_bar[stage]);
-      if (++stage == kStages) { stage = 0; phase ^= 1u; }
+      stage = nstage;
+      phase = nphase;
     }
 
     // ------------------------------- epilogue: registers -> global -------------------------------

@@ -139,6 +139,42 @@ def test_energy_sampled_triplets(cfg, count):
     assert np.all(got <= 0.0)
 
 
+@pytest.mark.parametrize("cfg", [4, 5])
+def test_full_size_bench_configuration_sampled(cfg):
+    """BASELINE.json configs[3], configs[4] at full array sizes, in the launch configuration
+    bench.py times (occupied window [0,10), automatic slab block and batch): sampled per-triplet
+    outputs (one i=j<k, one i<j=k, one i<j<k) against the oracle, plus the any-size properties."""
+    inp = make_config(cfg)
+    d = to_device(inp)
+    o = inp.nocc
+    opts = bqc.make_opts(occ_lo=0, occ_hi=10)
+    et = torch.empty(bqc.bqc_t_num_triplets(o), dtype=torch.float64, device="cuda")
+    e = bqc.bqc_t_energy_ex(*dims(inp), *d, opts=opts, e_triplet=et)
+    got = et.cpu().numpy()
+    assert abs(got.sum() - e) <= 1e-12 * abs(e)
+    inside = 0
+    for (i, j, k) in orc.triplet_list(10):
+        idx = bqc.bqc_t_triplet_index(o, i, j, k)
+        if i == j == k:
+            assert got[idx] == 0.0
+        else:
+            assert got[idx] < 0.0
+            inside += 1
+    assert inside == 210 and np.count_nonzero(got) == 210        # nothing outside the window
+    for (i, j, k) in [(2, 2, 7), (0, 9, 9), (1, 4, 8)]:
+        ref = orc.e_triplet(inp, i, j, k)
+        g = got[bqc.bqc_t_triplet_index(o, i, j, k)]
+        assert abs(g - ref) <= 1e-10 * abs(ref) + 1e-12 * abs(e) / 210, (i, j, k, g, ref)
+    # single W / V elements straight from Eq. (2) (6 + 6 dot products), ragged tail included
+    W, V = bqc.bqc_t_debug_wv(*dims(inp), *d, 1, 4, 8)
+    v = inp.nvir
+    scale = float(W.abs().max())
+    for (a, b, c) in [(0, 0, 0), (v - 1, v - 1, v - 1), (17, v - 1, 130), (255, 16, v - 3)]:
+        w_ref = orc.w_element(inp, 1, 4, 8, a, b, c)
+        assert abs(float(W[a, b, c]) - w_ref) <= 1e-11 * scale
+        assert abs(float(V[a, b, c]) - orc.v_element(inp, 1, 4, 8, a, b, c, w_ref)) <= 1e-11 * scale
+
+
 # ------------------------------------------------------------------ scheduler: windows, blocks, shards
 def test_blocking_window_and_sharding_agree_bitwise():
     inp = make_inputs(7, 20, 18, seed=41, t1_std=0.02)
