@@ -1,13 +1,15 @@
 // energy.cu — SURVEY.md §8(a) rows a3 + a4 (+ the reductions of a5).
 //
-// The W builder leaves, per triplet, three arrays in 16^3-blocked layout:
+// The W builder leaves, per triplet, three arrays in 8^3-blocked layout (each block a contiguous 4 KiB run):
 //     F1 = F(i,j,k)[a,b,c],  F2 = F(i,k,j)[a,c,b],  F3 = F(j,k,i)[b,c,a],   W[a,b,c] = F1 + F2 + F3
 // (see t_energy.cu).  The energy contraction needs W at all six index permutations of every point
-// (Eq. (3), reading G2), so a CTA owns one *orbit* of 16^3 tiles — the up-to-six tiles
+// (Eq. (3), reading G2), so a CTA owns one *orbit* of 8^3 tiles — the up-to-six tiles
 // reached from a block triple A <= B <= C by permutation — assembles the six W tiles in shared memory
-// (each F tile is read exactly once from HBM, as contiguous 32 KiB runs), forms V on the fly from the
-// (ov|ov) tiles and t1 (Eqs. (6),(7); V is never stored), and reduces
+// (each F tile is read exactly once from HBM), forms V on the fly from the (ov|ov) tiles and t1
+// (Eqs. (6),(7); V is never stored), and reduces
 //     sum_pi R_pi V_pi / D   (Eqs. (3),(4); the denominator is computed in registers, never stored).
+// 35 KB of shared memory and 256 threads per CTA: several CTAs per SM, so the HBM reads of one orbit
+// overlap the shared-memory and FP64 work of the others.
 // Reductions are fixed-order: warp shuffle tree -> per-CTA slot -> per-triplet sum -> final sum.
 #include "kernels.cuh"
 
@@ -15,23 +17,32 @@ namespace bqc {
 
 namespace {
 
-constexpr int kET = 16;
-constexpr int kEThreads = 512;
-constexpr int kTileElems = kET * kET * kET;   // 4096
+constexpr int kET = kVB;                      // 8
+constexpr int kEThreads = 256;
+constexpr int kTileElems = kET * kET * kET;   // 512
+constexpr int kJPitch = kET + 1;              // padded row pitch of the (ov|ov) tiles
+static_assert(kET == 8 && kEThreads == 256, "thread <-> element maps below assume 8^3 tiles and 256 threads");
 
 // the six permutations of three positions; 0-2 even (identity, two cyclic), 3-5 odd (transpositions)
 __device__ constexpr int kPerm[6][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}, {0, 2, 1}, {2, 1, 0}, {1, 0, 2}};
 // index of the ordered pair (s,t), s != t, in the (ov|ov) tile array
 __device__ constexpr int kPairIdx[3][3] = {{-1, 0, 1}, {2, -1, 3}, {4, 5, -1}};
 
-// XOR swizzle: consecutive lanes along ANY of the three tile axes fall into distinct columns of the
-// 128-byte row, so the transposed accumulations below and the permuted reads are conflict-free.
-__device__ __forceinline__ int sw(int x, int y, int z) { return (((x << 4) | y) << 4) | (z ^ x ^ y); }
+// Shared-memory position of tile element (X, Y, Z): linear index with its low 4 bits (the 8-byte bank
+// pair) XORed by a GF(2)-linear function of (X, Y>>1).  With this mask the 16 lanes of a half-warp hit 16
+// distinct bank pairs in every access pattern of the kernel: the three assembly passes (lanes vary along
+// w1,w2,v0,u0 of the F tile, written at (u,v,w), (u,w,v) and (w,u,v)) and the six permuted reads (lanes
+// vary along z and y0, read at every permutation of (x,y,z)).  The columns of the mask were found by
+// exhaustive search over all 2^20 linear maps.
+__device__ __forceinline__ int sw(int X, int Y, int Z) {
+  const int m = ((X & 1) * 9) ^ ((X & 2) << 1) ^ ((X & 4) >> 1) ^ ((Y & 2) << 1) ^ ((Y & 4) >> 1);
+  return ((X << 6) | (Y << 3) | Z) ^ m;
+}
 
 struct EnergySmem {
   double Wt[6][kTileElems];
-  double Jt[6][kET * kET];
-  double t1s[3][3][kET];   // [which occupied (i,j,k)][block position][local]
+  double Jt[3][6][kET * kJPitch];   // [m][ordered block-position pair][local u * pitch + local w]
+  double t1s[3][3][kET];            // [which occupied (i,j,k)][block position][local]
   double epsv[3][kET];
   double red[kEThreads / 32];
 };
@@ -42,80 +53,96 @@ __device__ __forceinline__ size_t blk_off(int nb, int P, int Q, int R) {
 
 }  // namespace
 
-__global__ void __launch_bounds__(kEThreads, 1) energy_kernel(const EnergyArgs a) {
-  extern __shared__ uint8_t esm_raw[];
-  EnergySmem& sm = *reinterpret_cast<EnergySmem*>(esm_raw);
+__global__ void __launch_bounds__(kEThreads, 3) energy_kernel(const EnergyArgs a) {
+  __shared__ EnergySmem sm;
   const int tid = threadIdx.x;
   const int orbit = blockIdx.x;
   const int tb = blockIdx.y;
   const int packed = a.orbits[orbit];
-  const int blk[3] = {packed & 255, (packed >> 8) & 255, (packed >> 16) & 255};
+  const int blk[3] = {packed & 1023, (packed >> 10) & 1023, (packed >> 20) & 1023};
   const TripletRec tr = a.trips[tb];
-  const int nb = a.nb16, v = a.v;
+  const int nb = a.nbv, v = a.v;
   const size_t fsz = (size_t)nb * nb * nb * kTileElems;
   const double* F1 = a.F + (size_t)tb * 3 * fsz;
   const double* F2 = F1 + fsz;
   const double* F3 = F2 + fsz;
 
-  // ---- small operands: t1 rows, virtual orbital energies
+  // ---- this thread's element pair of every F tile: tid bits (0..7) = (w1, w2, v0, u0, v1, v2, u1, u2)
+  const int ew = (tid & 3) << 1;
+  const int ev = ((tid >> 2) & 1) | (((tid >> 4) & 3) << 1);
+  const int eu = ((tid >> 3) & 1) | (((tid >> 6) & 3) << 1);
+  const int epair = ((eu << 6) | (ev << 3) | ew) >> 1;
+
+  auto load6 = [&](double2 (&val)[6], int phase) {
+#pragma unroll
+    for (int pi = 0; pi < 6; ++pi) {
+      const int P = blk[kPerm[pi][0]], Q = blk[kPerm[pi][1]], R = blk[kPerm[pi][2]];
+      const double* src = phase == 0 ? F1 + blk_off(nb, P, Q, R)
+                                     : (phase == 1 ? F2 + blk_off(nb, P, R, Q) : F3 + blk_off(nb, Q, R, P));
+      val[pi] = __ldg(reinterpret_cast<const double2*>(src) + epair);
+    }
+  };
+
+  double2 va[6], vb[6];
+  load6(va, 0);
+  load6(vb, 1);
+
+  // ---- small operands while the tile loads fly: t1 rows, virtual orbital energies, (ov|ov) tiles
   if (tid < 3 * 3 * kET) {
-    const int l = tid & 15, pos = (tid >> 4) % 3, which = tid / (3 * kET);
+    const int l = tid & 7, pos = (tid >> 3) % 3, which = tid / (3 * kET);
     const int occ = which == 0 ? tr.i : (which == 1 ? tr.j : tr.k);
     const int av = blk[pos] * kET + l;
     sm.t1s[which][pos][l] = (av < v) ? a.t1[(size_t)occ * v + av] : 0.0;
   } else if (tid < 3 * 3 * kET + 3 * kET) {
     const int e = tid - 3 * 3 * kET;
-    const int l = e & 15, pos = e >> 4;
+    const int l = e & 7, pos = e >> 3;
     const int av = blk[pos] * kET + l;
     sm.epsv[pos][l] = (av < v) ? a.eps_vir[av] : 1.0;
   }
-
-  // ---- assemble the six W tiles: W[a,b,c] = F1[a,b,c] + F2[a,c,b] + F3[b,c,a]
-  // thread -> element pairs L = 2*(tid + 512 r), (u, vv, w) = (L>>8, (L>>4)&15, L&15), w even
-#pragma unroll 1
-  for (int phase = 0; phase < 3; ++phase) {
-#pragma unroll 1
-    for (int half = 0; half < 2; ++half) {
-      double2 val[3][4];
-#pragma unroll
-      for (int pp = 0; pp < 3; ++pp) {
-        const int pi = half * 3 + pp;
-        const int P = blk[kPerm[pi][0]], Q = blk[kPerm[pi][1]], R = blk[kPerm[pi][2]];
-        const double* src = phase == 0 ? F1 + blk_off(nb, P, Q, R)
-                                       : (phase == 1 ? F2 + blk_off(nb, P, R, Q) : F3 + blk_off(nb, Q, R, P));
-#pragma unroll
-        for (int r = 0; r < 4; ++r)
-          val[pp][r] = __ldg(reinterpret_cast<const double2*>(src) + tid + kEThreads * r);
-      }
-#pragma unroll
-      for (int pp = 0; pp < 3; ++pp) {
-        double* W = sm.Wt[half * 3 + pp];
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-          const int L = 2 * (tid + kEThreads * r);
-          const int u = L >> 8, vv = (L >> 4) & 15, w = L & 15;
-          if (phase == 0) {          // F1 tile [x][y][z] = (u, vv, w)
-            W[sw(u, vv, w)] = val[pp][r].x;
-            W[sw(u, vv, w + 1)] = val[pp][r].y;
-          } else if (phase == 1) {   // F2 tile [x][z][y] = (u, vv, w)
-            W[sw(u, w, vv)] += val[pp][r].x;
-            W[sw(u, w + 1, vv)] += val[pp][r].y;
-          } else {                   // F3 tile [y][z][x] = (u, vv, w)
-            W[sw(w, u, vv)] += val[pp][r].x;
-            W[sw(w + 1, u, vv)] += val[pp][r].y;
-          }
-        }
-      }
+  if (a.use_t1) {
+    for (int e = tid; e < 3 * 6 * kET * kET; e += kEThreads) {
+      const int lw = e & 7, lu = (e >> 3) & 7, pr = (e >> 6) % 6, m = e / (6 * kET * kET);
+      // J^(0) = J_jk, J^(1) = J_ik, J^(2) = J_ij
+      const int px = (m == 0) ? tr.pj : tr.pi;
+      const int py = (m == 2) ? tr.pj : tr.pk;
+      const double* Jm = a.J + ((size_t)px * a.nw + py) * v * v;
+      // pair index -> ordered block positions (s, t)
+      const int s = pr >> 1;
+      const int t = (pr & 1) ? (s == 2 ? 1 : 2) : (s == 0 ? 1 : 0);
+      const int gu = blk[s] * kET + lu, gw = blk[t] * kET + lw;
+      sm.Jt[m][pr][lu * kJPitch + lw] = (gu < v && gw < v) ? __ldg(Jm + (size_t)gu * v + gw) : 0.0;
     }
-    __syncthreads();
   }
 
-  // ---- points of this thread: z = tid & 15, y = (tid >> 4) & 15, x = (tid >> 8) + 2 r
-  const int lz = tid & 15, ly = (tid >> 4) & 15, lx0 = tid >> 8;
-  double num[8];
+  // ---- assemble the six W tiles: W[x,y,z] = F1[x,y,z] + F2[x,z,y] + F3[y,z,x]
+  // (F tile element (eu, ev, ew): F1 -> (x,y,z), F2 -> (x,z,y), F3 -> (y,z,x))
 #pragma unroll
-  for (int r = 0; r < 8; ++r) {
-    const int l[3] = {lx0 + 2 * r, ly, lz};
+  for (int pi = 0; pi < 6; ++pi) {
+    sm.Wt[pi][sw(eu, ev, ew)] = va[pi].x;
+    sm.Wt[pi][sw(eu, ev, ew + 1)] = va[pi].y;
+  }
+  __syncthreads();
+  load6(va, 2);
+#pragma unroll
+  for (int pi = 0; pi < 6; ++pi) {
+    sm.Wt[pi][sw(eu, ew, ev)] += vb[pi].x;
+    sm.Wt[pi][sw(eu, ew + 1, ev)] += vb[pi].y;
+  }
+  __syncthreads();
+#pragma unroll
+  for (int pi = 0; pi < 6; ++pi) {
+    sm.Wt[pi][sw(ew, eu, ev)] += va[pi].x;
+    sm.Wt[pi][sw(ew + 1, eu, ev)] += va[pi].y;
+  }
+  __syncthreads();
+
+  // ---- points of this thread: z = tid & 7, y = (tid >> 3) & 7, x = (tid >> 6) + 4 r
+  const int lz = tid & 7, ly = (tid >> 3) & 7, lx0 = tid >> 6;
+  const double dijk = a.eps_occ[tr.i] + a.eps_occ[tr.j] + a.eps_occ[tr.k];
+  double acc = 0.0;
+#pragma unroll
+  for (int r = 0; r < 2; ++r) {
+    const int l[3] = {lx0 + 4 * r, ly, lz};
     double w[6];
 #pragma unroll
     for (int p = 0; p < 6; ++p) w[p] = sm.Wt[p][sw(l[kPerm[p][0]], l[kPerm[p][1]], l[kPerm[p][2]])];
@@ -123,57 +150,24 @@ __global__ void __launch_bounds__(kEThreads, 1) energy_kernel(const EnergyArgs a
     const double re = se - 2.0 * so, ro = so - 2.0 * se;
     double s = 0.0;
 #pragma unroll
-    for (int p = 0; p < 6; ++p) s += (3.0 * w[p] + (p < 3 ? re : ro)) * w[p];
-    num[r] = s;
-  }
-
-  if (a.use_t1) {
-#pragma unroll 1
-    for (int m = 0; m < 3; ++m) {
-      // J^(0) = J_jk, J^(1) = J_ik, J^(2) = J_ij
-      const int px = (m == 0) ? tr.pj : tr.pi;
-      const int py = (m == 2) ? tr.pj : tr.pk;
-      const double* Jm = a.J + ((size_t)px * a.nw + py) * v * v;
-      __syncthreads();
-      for (int e = tid; e < 6 * kET * kET; e += kEThreads) {
-        const int lw = e & 15, lu = (e >> 4) & 15, pr = e >> 8;
-        // pair index -> ordered block positions (s, t)
-        const int s = pr >> 1;
-        const int t = (pr & 1) ? (s == 2 ? 1 : 2) : (s == 0 ? 1 : 0);
-        const int gu = blk[s] * kET + lu, gw = blk[t] * kET + lw;
-        sm.Jt[pr][(lu << 4) | lw] = (gu < v && gw < v) ? __ldg(Jm + (size_t)gu * v + gw) : 0.0;
-      }
-      __syncthreads();
-      const int sA = (m == 0) ? 1 : 0, sB = (m == 2) ? 1 : 2;
+    for (int p = 0; p < 6; ++p) {
+      // V at the permuted point: W + t1[i,a](jb|kc) + t1[j,b](ia|kc) + t1[k,c](ia|jb)   (Eqs. (6),(7))
+      double vp = w[p];
+      if (a.use_t1) {
 #pragma unroll
-      for (int r = 0; r < 8; ++r) {
-        const int l[3] = {lx0 + 2 * r, ly, lz};
-        double w[6];
-#pragma unroll
-        for (int p = 0; p < 6; ++p) w[p] = sm.Wt[p][sw(l[kPerm[p][0]], l[kPerm[p][1]], l[kPerm[p][2]])];
-        const double se = w[0] + w[1] + w[2], so = w[3] + w[4] + w[5];
-        const double re = se - 2.0 * so, ro = so - 2.0 * se;
-        double s = 0.0;
-#pragma unroll
-        for (int p = 0; p < 6; ++p) {
+        for (int m = 0; m < 3; ++m) {
+          const int sA = (m == 0) ? 1 : 0, sB = (m == 2) ? 1 : 2;
           const int pm = kPerm[p][m], pa = kPerm[p][sA], pb = kPerm[p][sB];
-          const double x = sm.t1s[m][pm][l[pm]] * sm.Jt[kPairIdx[pa][pb]][(l[pa] << 4) | l[pb]];
-          s += (3.0 * w[p] + (p < 3 ? re : ro)) * x;
+          vp = fma(sm.t1s[m][pm][l[pm]], sm.Jt[m][kPairIdx[pa][pb]][l[pa] * kJPitch + l[pb]], vp);
         }
-        num[r] += s;
       }
+      // R at the permuted point = 3 w_p + (sum of same-parity w) - 2 (sum of opposite-parity w)   (Eq. (3))
+      s += (3.0 * w[p] + (p < 3 ? re : ro)) * vp;
     }
-  }
-
-  // ---- denominators (Eq. (3)), in registers
-  const double dijk = a.eps_occ[tr.i] + a.eps_occ[tr.j] + a.eps_occ[tr.k];
-  double acc = 0.0;
-#pragma unroll
-  for (int r = 0; r < 8; ++r) {
-    const int lx = lx0 + 2 * r;
-    const bool valid = (blk[0] * kET + lx < v) && (blk[1] * kET + ly < v) && (blk[2] * kET + lz < v);
-    const double d = dijk - sm.epsv[0][lx] - sm.epsv[1][ly] - sm.epsv[2][lz];
-    if (valid) acc += num[r] / d;
+    // denominator (Eq. (3)) in registers
+    const bool valid = (blk[0] * kET + l[0] < v) && (blk[1] * kET + ly < v) && (blk[2] * kET + lz < v);
+    const double d = dijk - sm.epsv[0][l[0]] - sm.epsv[1][ly] - sm.epsv[2][lz];
+    if (valid) acc += s / d;
   }
   // multiplicity of the block triple under permutation (1, 2 or 6)
   const int same = (blk[0] == blk[1]) + (blk[1] == blk[2]);
@@ -193,15 +187,9 @@ __global__ void __launch_bounds__(kEThreads, 1) energy_kernel(const EnergyArgs a
 }
 
 int launch_energy(const EnergyArgs& a, cudaStream_t s) {
-  static bool attr_set = false;
-  if (!attr_set) {
-    BQC_CUDA_OK(cudaFuncSetAttribute(energy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)sizeof(EnergySmem)));
-    attr_set = true;
-  }
   if (a.ntrip <= 0) return BQC_OK;
   dim3 grid(a.norbits, a.ntrip);
-  energy_kernel<<<grid, kEThreads, sizeof(EnergySmem), s>>>(a);
+  energy_kernel<<<grid, kEThreads, 0, s>>>(a);
   count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
@@ -272,7 +260,7 @@ __global__ void assemble_wv_kernel(const double* __restrict__ F, int nb, int v, 
     const int b = (int)((e / v) % v);
     const int a = (int)(e / ((long long)v * v));
     auto at = [&](const double* Fx, int p, int q, int r) {
-      return Fx[blk_off(nb, p >> 4, q >> 4, r >> 4) + ((((p & 15) << 4) | (q & 15)) << 4 | (r & 15))];
+      return Fx[blk_off(nb, p >> 3, q >> 3, r >> 3) + ((((p & 7) << 3) | (q & 7)) << 3 | (r & 7))];
     };
     const double w = at(F, a, b, c) + at(F + fsz, a, c, b) + at(F + 2 * fsz, b, c, a);
     if (W) W[e] = w;
@@ -282,11 +270,11 @@ __global__ void assemble_wv_kernel(const double* __restrict__ F, int nb, int v, 
   }
 }
 
-int launch_assemble_wv(const double* F, int nb16, int v, const double* J, int nw, int pi, int pj, int pk,
+int launch_assemble_wv(const double* F, int nbv, int v, const double* J, int nw, int pi, int pj, int pk,
                        const double* t1i, const double* t1j, const double* t1k, double* W, double* V,
                        cudaStream_t s) {
   const size_t v2 = (size_t)v * v;
-  assemble_wv_kernel<<<1024, 256, 0, s>>>(F, nb16, v, J + ((size_t)pj * nw + pk) * v2,
+  assemble_wv_kernel<<<1024, 256, 0, s>>>(F, nbv, v, J + ((size_t)pj * nw + pk) * v2,
                                           J + ((size_t)pi * nw + pk) * v2, J + ((size_t)pi * nw + pj) * v2,
                                           t1i, t1j, t1k, W, V);
   count_launch();

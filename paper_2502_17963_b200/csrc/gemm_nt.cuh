@@ -55,10 +55,10 @@ struct GemmParams {
   int m1_ext, m2_ext, n_ext;         // valid extents of the output index ranges
   int kiters;                        // ceil(K / 16) per term
   // output addressing
-  int out_mode;                      // 0: strided, 1: blocked 16^3 tiles (F layout)
+  int out_mode;                      // 0: strided, 1: blocked 8^3 tiles (F layout)
   int n2_ext;                        // strided: n -> (n / n2_ext, n % n2_ext)
   long long sM1, sM2, sN1, sN2;      // strided: off = c_off + m1*sM1 + m2*sM2 + n1*sN1 + n2*sN2
-  int nb16;                          // blocked: blocks per dimension
+  int nbv;                           // blocked: 8-blocks per dimension
   const GemmTask* tasks;
   double* C;
 };
@@ -237,8 +237,8 @@ gemm_nt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         const bool has1 = (n + 1) < prm.n_ext;
         if (prm.out_mode == 1) {
           const long long off =
-              ((((long long)(m1 >> 4) * prm.nb16 + (m2 >> 4)) * prm.nb16 + (n >> 4)) << 12) +
-              ((((m1 & 15) << 4) + (m2 & 15)) << 4) + (n & 15);
+              ((((long long)(m1 >> 3) * prm.nbv + (m2 >> 3)) * prm.nbv + (n >> 3)) << 9) +
+              ((((m1 & 7) << 3) + (m2 & 7)) << 3) + (n & 7);
           if (has1) {
             *reinterpret_cast<double2*>(C + off) = make_double2(acc[i][j][0], acc[i][j][1]);
           } else {

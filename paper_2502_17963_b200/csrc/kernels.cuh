@@ -15,6 +15,9 @@ int launch_btilde_t2(const double* t2, double* btil, int o, int v, const int* ac
 int launch_slab_holes(const double* t2, double* slabs, int o, int v, int kp, int x0, int nx,
                       int slot0, cudaStream_t s);
 
+// Edge of the cubic virtual-index blocks of the F layout (GEMM epilogue writes, energy kernel reads).
+constexpr int kVB = 8;
+
 // One entry per triplet of a batch.
 struct TripletRec {
   int i, j, k;        // occupied indices, i <= j <= k
@@ -23,15 +26,15 @@ struct TripletRec {
 };
 
 struct EnergyArgs {
-  const double* F;          // [ntrip][3][nb16^3][16^3] blocked F(i,j,k), F(i,k,j), F(j,k,i)
+  const double* F;          // [ntrip][3][nbv^3][8^3] blocked F(i,j,k), F(i,k,j), F(j,k,i)
   const TripletRec* trips;  // [ntrip]
-  const int* orbits;        // [norbits] packed A | B<<8 | C<<16, A <= B <= C
+  const int* orbits;        // [norbits] packed A | B<<10 | C<<20, A <= B <= C
   const double* J;          // [nw*nw][v][v]   J_xy[u,w] = (xu|yw)
   const double* t1;         // [o][v]
   const double* eps_occ;    // [o]
   const double* eps_vir;    // [v]
   double* partial;          // [ntrip][norbits]
-  int ntrip, norbits, nb16, v, nw, use_t1;
+  int ntrip, norbits, nbv, v, nw, use_t1;
 };
 int launch_energy(const EnergyArgs& a, cudaStream_t s);
 
@@ -42,7 +45,7 @@ int launch_reduce_triplets(const double* partial, const TripletRec* trips, int n
 int launch_final_sum(const double* e_trip, long long n, double* out, cudaStream_t s);
 
 // dense W / V [v][v][v] of one triplet from its three blocked F arrays (debug / parity of rows a2, a3)
-int launch_assemble_wv(const double* F, int nb16, int v, const double* J, int nw, int pi, int pj, int pk,
+int launch_assemble_wv(const double* F, int nbv, int v, const double* J, int nw, int pi, int pj, int pk,
                        const double* t1i, const double* t1j, const double* t1k, double* W, double* V,
                        cudaStream_t s);
 

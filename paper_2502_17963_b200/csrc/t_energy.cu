@@ -49,7 +49,7 @@ struct Plan {
   std::vector<int> act;        // active occupied orbitals (sorted); triplets are drawn from these
   int na = 0;                  // act.size()
   int Xp = 0, Kp = 0;          // aux / (v+o) extents padded to multiples of 16
-  int nb16 = 0;                // 16-blocks per virtual dimension
+  int nbv = 0;                 // 8-blocks per virtual dimension
   size_t fsz = 0;              // doubles per blocked F array
   size_t slab_elems = 0;       // v*v*Kp
   int Bo = 0, nblk = 0, nsets = 0, nslots = 0;
@@ -108,10 +108,10 @@ int make_plan(Plan& P, int o, int v, int X, const std::vector<int>& act, const b
   P.na = (int)act.size();
   P.Xp = round_up_i(X, 16);
   P.Kp = round_up_i(v + o, 16);
-  P.nb16 = ceil_div(v, 16);
-  P.fsz = (size_t)P.nb16 * P.nb16 * P.nb16 * 4096;
+  P.nbv = ceil_div(v, kVB);
+  P.fsz = (size_t)P.nbv * P.nbv * P.nbv * (kVB * kVB * kVB);
   P.slab_elems = (size_t)v * v * P.Kp;
-  P.norbits = P.nb16 * (P.nb16 + 1) * (P.nb16 + 2) / 6;
+  P.norbits = (int)((long long)P.nbv * (P.nbv + 1) * (P.nbv + 2) / 6);
   P.use_t1 = !(opts && (opts->flags & BQC_T_FLAG_NO_T1));
   P.profile = (opts && (opts->flags & BQC_T_FLAG_PROFILE)) ? 1 : 0;
   P.shard_count = (opts && opts->shard_count > 0) ? opts->shard_count : 1;
@@ -171,7 +171,7 @@ int check_sizes(int o, int v, int X) {
     set_error(BQC_ERR_INVALID_SIZE, "nocc=%d nvir=%d naux=%d must all be > 0", o, v, X);
     return BQC_ERR_INVALID_SIZE;
   }
-  if (v > 255 * 16 || o > 4096) {
+  if (v > 1023 * kVB || o > 4096) {
     set_error(BQC_ERR_INVALID_SIZE, "nocc=%d nvir=%d exceed the supported range", o, v);
     return BQC_ERR_INVALID_SIZE;
   }
@@ -436,9 +436,9 @@ int Pipeline::prepare() {
   {
     std::vector<int> orb;
     orb.reserve(P.norbits);
-    for (int A = 0; A < P.nb16; ++A)
-      for (int B = A; B < P.nb16; ++B)
-        for (int C = B; C < P.nb16; ++C) orb.push_back(A | (B << 8) | (C << 16));
+    for (int A = 0; A < P.nbv; ++A)
+      for (int B = A; B < P.nbv; ++B)
+        for (int C = B; C < P.nbv; ++C) orb.push_back(A | (B << 10) | (C << 20));
     BQC_CUDA_OK(cudaMemcpyAsync(c.orbits_dev(), orb.data(), orb.size() * 4, cudaMemcpyHostToDevice, s));
     BQC_CUDA_OK(cudaStreamSynchronize(s));   // `orb` goes out of scope
   }
@@ -617,7 +617,7 @@ int Pipeline::compute(const Action& a) {
   prm.m1_ext = v; prm.m2_ext = v; prm.n_ext = v;
   prm.kiters = P.Kp / kBK;
   prm.out_mode = 1;
-  prm.nb16 = P.nb16;
+  prm.nbv = P.nbv;
   prm.n2_ext = 1;
   prm.tasks = c.tasks_dev() + a.task0;
   prm.C = c.F();
@@ -629,7 +629,7 @@ int Pipeline::compute(const Action& a) {
   e.F = c.F(); e.trips = c.trips_dev() + a.trip0; e.orbits = c.orbits_dev();
   e.J = c.J(); e.t1 = c.in.t1; e.eps_occ = c.in.eps_occ; e.eps_vir = c.in.eps_vir;
   e.partial = c.partial();
-  e.ntrip = (int)a.ntrip; e.norbits = P.norbits; e.nb16 = P.nb16; e.v = v; e.nw = P.na; e.use_t1 = P.use_t1;
+  e.ntrip = (int)a.ntrip; e.norbits = P.norbits; e.nbv = P.nbv; e.v = v; e.nw = P.na; e.use_t1 = P.use_t1;
   BQC_TRY(launch_energy(e, s));
   BQC_TRY(launch_reduce_triplets(c.partial(), c.trips_dev() + a.trip0, (int)a.ntrip, P.norbits, c.etrip(), s));
   if (P.profile) BQC_TRY(c.prof_mark(c.prof_main, s));
@@ -1047,12 +1047,12 @@ int bqc_t_debug_wv(int nocc, int nvir, int naux, const double* eps_occ, const do
   prm.m1_ext = nvir; prm.m2_ext = nvir; prm.n_ext = nvir;
   prm.kiters = P.Kp / kBK;
   prm.out_mode = 1;
-  prm.nb16 = P.nb16;
+  prm.nbv = P.nbv;
   prm.n2_ext = 1;
   prm.tasks = c.tasks_dev() + task0;
   prm.C = c.F();
   BQC_TRY(launch_gemm_nt(c.f_nf, c.tm_slab, c.tm_slabT, c.tm_btil, prm, stream));
-  BQC_TRY(launch_assemble_wv(c.F(), P.nb16, nvir, c.J(), P.na, pi, pj, pk, t1 + (size_t)i * nvir,
+  BQC_TRY(launch_assemble_wv(c.F(), P.nbv, nvir, c.J(), P.na, pi, pj, pk, t1 + (size_t)i * nvir,
                              t1 + (size_t)j * nvir, t1 + (size_t)k * nvir, W_dev, V_dev, stream));
   BQC_CUDA_OK(cudaStreamSynchronize(stream));
   BQC_CUDA_OK(cudaStreamSynchronize(c.s_form));
