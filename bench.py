@@ -49,6 +49,7 @@ def parse():
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--peak-seconds", type=float, default=2.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-triplets", type=int, default=3, help="triplets the oracle evaluates (cpu_baseline)")
     return ap.parse_args()
 
 
@@ -217,8 +218,10 @@ def main():
     # FP64 tensor-core peak measured in this run: the roofline denominator
     peak_dmma = bqc.bqc_fp64_peak_tflops(0, args.peak_seconds)
 
+    e_trip = torch.zeros(bqc.bqc_t_num_triplets(o), dtype=torch.float64, device="cuda")
+
     def step():
-        return bqc.bqc_t_energy_ex(o, v, X, *dev, opts=opts, workspace=ws)
+        return bqc.bqc_t_energy_ex(o, v, X, *dev, opts=opts, workspace=ws, e_triplet=e_trip)
 
     for _ in range(args.warmup):
         e_val = step()
@@ -306,12 +309,26 @@ def main():
             "gpu_launches": launches,
         }
         if world == 1 and not args.no_cpu_baseline:
-            trip = (lo, (lo + hi - 1) // 2, hi - 1)
-            dt, e_ref = oracle_sample(inp, trip)
+            # the oracle as it stands on three triplets of the workload (one per class i<j<k, i=j<k, i<j=k); its
+            # per-triplet values are compared with the e_ijk the timed GPU steps produced (north_star tolerance)
+            mid = (lo + hi - 1) // 2
+            trips = [(lo, mid, hi - 1), (lo, lo, hi - 1), (lo, hi - 1, hi - 1)][:max(1, args.cpu_triplets)]
             f1 = 12.0 * v ** 3 * (v + o)
-            out["cpu_baseline"] = {"value": f1 / dt * 1e-12, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
-                                   "sample": f"one triplet {trip} of the workload ({f1:.3e} flops) in {dt:.1f} s, "
-                                             "NumPy/OpenBLAS oracle as it stands"}
+            e_gpu = e_trip.cpu().numpy()
+            dts, worst = [], 0.0
+            for trip in trips:
+                dt, e_ref = oracle_sample(inp, trip)
+                dts.append(dt)
+                d = abs(e_gpu[bqc.bqc_t_triplet_index(o, *trip)] - e_ref)
+                worst = max(worst, d / (1e-10 * abs(e_ref) + 1e-12 * abs(e_total) / max(ntrip, 1)))
+            dt = float(np.sum(dts))
+            out["cpu_baseline"] = {"value": len(trips) * f1 / dt * 1e-12, "unit": UNIT, "cores": cpu_threads(),
+                                   "kind": "oracle",
+                                   "sample": f"triplets {trips} of the workload ({f1:.3e} flops each) in {dt:.1f} s, "
+                                             "NumPy/OpenBLAS oracle as it stands",
+                                   "seconds_per_full_E_T_extrapolated": dt / len(trips) * flops_full / f1,
+                                   "gpu_vs_oracle_worst_err_over_tol": worst}
+            assert worst <= 1.0, f"GPU per-triplet energies differ from the oracle: {worst:.3g} x tolerance"
         print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -11,7 +11,9 @@ Recipe (BASELINE.json `configs`, reading G12 of SURVEY.md §8(c)):
     3. ``eps_vir`` [nvir] uniform[0.15, 3.0], sorted ascending;
     4. ``t1``    [nocc, nvir] N(0, t1_std);
     5. ``G_t2``  [nocc, nocc, nvir, nvir] N(0, t2_std),
-       ``t2 = (G_t2 + G_t2.transpose(1, 0, 3, 2)) / 2``.
+       ``t2 = (G_t2 + G_t2.transpose(1, 0, 3, 2)) / 2``;
+    6. only when ``f_std > 0`` (non-canonical reference):
+       ``f_ov`` [nocc, nvir] N(0, f_std), drawn last so draws 1-5 do not change.
 * integrals are *defined* as (pq|rs) = sum_Q B[Q,p,q] B[Q,r,s]  (exact DF).
 
 These are synthetic stand-ins shaped like the paper's water-cluster cc-pVDZ
@@ -38,6 +40,7 @@ class TInputs:
     B_ov: np.ndarray      # [naux, nocc, nvir]
     B_vv: np.ndarray      # [naux, nvir, nvir]
     name: str = ""
+    f_ov: np.ndarray | None = None   # [nocc, nvir] occupied-virtual Fock block; None = canonical RHF
 
     def arrays(self):
         return (self.eps_occ, self.eps_vir, self.t1, self.t2,
@@ -59,7 +62,7 @@ CONFIGS = {
 
 def make_inputs(nocc: int, nvir: int, naux: int, seed: int,
                 t1_std: float = 1e-3, t2_std: float = 1e-2,
-                b_std: float = 0.1, name: str = "") -> TInputs:
+                b_std: float = 0.1, name: str = "", f_std: float = 0.0) -> TInputs:
     """Generate one seeded input set following the G12 recipe above."""
     rng = np.random.default_rng(seed)
     n = nocc + nvir
@@ -90,8 +93,9 @@ def make_inputs(nocc: int, nvir: int, naux: int, seed: int,
                 a += b.T
                 a *= 0.5
                 b[...] = a.T
+    f_ov = rng.normal(0.0, f_std, size=(nocc, nvir)) if f_std > 0.0 else None
     return TInputs(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv,
-                   name=name or f"o{nocc}v{nvir}x{naux}s{seed}")
+                   name=name or f"o{nocc}v{nvir}x{naux}s{seed}", f_ov=f_ov)
 
 
 def make_config(idx: int, **overrides) -> TInputs:
@@ -100,7 +104,7 @@ def make_config(idx: int, **overrides) -> TInputs:
     c.update(overrides)
     return make_inputs(c["nocc"], c["nvir"], c["naux"], c["seed"],
                        t1_std=c.get("t1_std", 1e-3), t2_std=c["t2_std"],
-                       name=f"config{idx}")
+                       name=f"config{idx}", f_std=c.get("f_std", 0.0))
 
 
 def worked_example(nocc: int, nvir: int, naux: int) -> TInputs:

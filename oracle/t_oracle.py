@@ -26,7 +26,9 @@ PAPER.md:288-305 (§2.4.2, Eqs. (2)-(7)) with the readings G1-G7 of SURVEY.md
 
 Integrals are exact density fitting, (pq|rs) = sum_Q B[Q,p,q] B[Q,r,s]
 (BASELINE.json configs[0]).  The Fock term of Eqs. (5),(7)
-vanishes for canonical RHF (G7).
+vanishes for canonical RHF (G7); when the input carries an occupied-virtual
+Fock block ``f_ov`` V gains
+f[i,a] t2[j,k,b,c] + f[j,b] t2[i,k,a,c] + f[k,c] t2[i,j,a,b]  (reading G15).
 
 Arithmetic is FP64 NumPy.  ``numpy.einsum`` / ``@`` serve as the library
 contraction primitive of each step; there is no blocking, fusion or reordering
@@ -88,12 +90,22 @@ def w_triplet(inp, i, j, k, slabs=None):
 
 
 def v_triplet(inp, i, j, k, W):
-    """V = W + t1 (ov|ov) terms (Eqs. (6),(7), reading G6)."""
+    """V = W + t1 (ov|ov) terms (Eqs. (6),(7), reading G6).
+
+    Non-canonical reference (inp.f_ov given; Eqs. (5),(7), reading G15): the x-term
+    x_k F_ck = 0.5 P sum_ij t_ij^ab v_ijk F_ck adds, by the same argument as G6,
+    f[i,a] t2[j,k,b,c] + f[j,b] t2[i,k,a,c] + f[k,c] t2[i,j,a,b] to V.
+    """
     t1 = inp.t1
     V = W.copy()
     V += t1[i][:, None, None] * slab_ovov(inp, j, k)[None, :, :]
     V += t1[j][None, :, None] * slab_ovov(inp, i, k)[:, None, :]
     V += t1[k][None, None, :] * slab_ovov(inp, i, j)[:, :, None]
+    f = getattr(inp, "f_ov", None)
+    if f is not None:
+        V += f[i][:, None, None] * inp.t2[j, k][None, :, :]
+        V += f[j][None, :, None] * inp.t2[i, k][:, None, :]
+        V += f[k][None, None, :] * inp.t2[i, j][:, :, None]
     return V
 
 
@@ -188,4 +200,9 @@ def v_element(inp, i, j, k, a, b, c, w=None):
     jbkc = float(B[:, j, b] @ B[:, k, c])
     iakc = float(B[:, i, a] @ B[:, k, c])
     iajb = float(B[:, i, a] @ B[:, j, b])
-    return w + inp.t1[i, a] * jbkc + inp.t1[j, b] * iakc + inp.t1[k, c] * iajb
+    val = w + inp.t1[i, a] * jbkc + inp.t1[j, b] * iakc + inp.t1[k, c] * iajb
+    f = getattr(inp, "f_ov", None)
+    if f is not None:
+        val += (f[i, a] * inp.t2[j, k, b, c] + f[j, b] * inp.t2[i, k, a, c]
+                + f[k, c] * inp.t2[i, j, a, b])
+    return val

@@ -11,6 +11,9 @@ Jordan-Wigner matrices on the full Fock space of 2(o+v) spin orbitals;
     R3    = diag(1/D) on triply excited determinants, D = sum eps_holes - sum eps_particles
     E[4]  = <0| T2+ W_N R3 W_N T2 |0>,   E[5] = <0| T1+ W_N R3 W_N T2 |0>,
     E(T)  = E[4] + E[5]
+Non-canonical reference (Eqs. (5),(7)): with an occupied-virtual
+Fock block f_ov the fluctuation potential gains the one-body operator F_ov = sum_ia f[i,a] (E_ia + E_ai) and
+    E[F]  = <0| T2+ F_ov R3 W_N T2 |0>,   E(T) = E[4] + E[5] + E[F].
 (textbook CCSD(T): Raghavachari et al. 1989; the closed-shell index formula the
 paper optimises, PAPER.md:288 ref. 62, must reproduce these numbers.)
 """
@@ -31,8 +34,8 @@ def _jw_annihilators(nso):
     return ops
 
 
-def first_principles_t(inp):
-    """Return (E4, E5) for a TInputs; feasible for o+v <= 7."""
+def first_principles_t(inp, with_fock=False):
+    """Return (E4, E5) — or (E4, E5, EF) with `with_fock` — for a TInputs; feasible for o+v <= 7."""
     o, v = inp.nocc, inp.nvir
     n = o + v
     nso = 2 * n
@@ -105,4 +108,11 @@ def first_principles_t(inp):
                 D -= eps[p]
         if holes == 3 and parts == 3:
             r3[d] = 1.0 / D
-    return float(psi @ (r3 * psi)), float(phi @ (r3 * psi))
+    e4, e5 = float(psi @ (r3 * psi)), float(phi @ (r3 * psi))
+    if not with_fock:
+        return e4, e5
+    chi = np.zeros(dim)
+    for i in range(o):
+        for aa in range(v):
+            chi += inp.f_ov[i, aa] * ((E[o + aa][i] + E[i][o + aa]) @ t2v)
+    return e4, e5, float(chi @ (r3 * psi))

@@ -268,3 +268,43 @@ def test_sample_triplets_cover_classes():
     assert all(i <= j <= k for i, j, k in s)
     assert any(i == j < k for i, j, k in s) and any(i < j == k for i, j, k in s)
     assert any(i < j < k for i, j, k in s) and any(i == j == k for i, j, k in s)
+
+
+# ---- NEXT-3: occupied-virtual Fock block (Eqs. (5),(7)) ----
+def test_fock_term_is_linear_in_f_and_vanishes_at_zero():
+    inp = make_inputs(3, 5, 7, seed=21, t1_std=0.05, t2_std=0.05, f_std=0.1)
+    canon = copy.copy(inp); canon.f_ov = None
+    zero = copy.copy(inp); zero.f_ov = np.zeros_like(inp.f_ov)
+    twice = copy.copy(inp); twice.f_ov = 2.0 * inp.f_ov
+    e0, e1, e2 = orc.t_energy(canon), orc.t_energy(inp), orc.t_energy(twice)
+    assert orc.t_energy(zero) == e0
+    assert abs(e1 - e0) > 1e-6 * abs(e0)
+    assert (e2 - e0) == pytest.approx(2.0 * (e1 - e0), rel=1e-10)
+    # E_F is bilinear in (f, t2) x (W ~ t2): scaling t2 by s scales it by s^2, t1 does not enter it
+    not1 = copy.copy(inp); not1.t1 = np.zeros_like(inp.t1)
+    not1c = copy.copy(canon); not1c.t1 = np.zeros_like(inp.t1)
+    assert (orc.t_energy(not1) - orc.t_energy(not1c)) == pytest.approx(e1 - e0, rel=1e-10)
+
+
+def test_fock_term_brute_force_and_elements():
+    """E_F against a dense six-index contraction sum_{ijkabc} R[W] f[k,c] t2[i,j,a,b] / D (x3 by symmetry / 3)."""
+    inp = make_inputs(3, 4, 6, seed=22, t1_std=0.05, t2_std=0.05, f_std=0.1)
+    canon = copy.copy(inp); canon.f_ov = None
+    o, v = inp.nocc, inp.nvir
+    W6 = np.zeros((o, o, o, v, v, v))
+    for i, j, k in itertools.product(range(o), repeat=3):
+        W6[i, j, k] = orc.w_triplet(inp, i, j, k)
+    R6 = (4 * W6 + W6.transpose(0, 1, 2, 4, 5, 3) + W6.transpose(0, 1, 2, 5, 3, 4)
+          - 2 * (W6.transpose(0, 1, 2, 3, 5, 4) + W6.transpose(0, 1, 2, 5, 4, 3) + W6.transpose(0, 1, 2, 4, 3, 5)))
+    eo, ev = inp.eps_occ, inp.eps_vir
+    D6 = (eo[:, None, None, None, None, None] + eo[None, :, None, None, None, None]
+          + eo[None, None, :, None, None, None] - ev[None, None, None, :, None, None]
+          - ev[None, None, None, None, :, None] - ev[None, None, None, None, None, :])
+    # the three f*t2 terms are images of one another under simultaneous (occ, vir) relabelling, and R/D is
+    # invariant under it: (1/3) sum_all 3 * [R/D * f[k,c] t2[i,j,a,b]]
+    ef = np.einsum("ijkabc,kc,ijab->", R6 / D6, inp.f_ov, inp.t2)
+    assert (orc.t_energy(inp) - orc.t_energy(canon)) == pytest.approx(ef, rel=1e-10)
+    W = orc.w_triplet(inp, 0, 1, 2)
+    V = orc.v_triplet(inp, 0, 1, 2, W)
+    for (a, b, c) in [(0, 1, 2), (3, 3, 1), (2, 0, 0)]:
+        assert orc.v_element(inp, 0, 1, 2, a, b, c) == pytest.approx(V[a, b, c], rel=1e-11, abs=1e-16)
