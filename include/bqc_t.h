@@ -8,6 +8,8 @@
  *   W_ijk[abc]  = P sum_d (ia|bd) t2[k,j,c,d] - P sum_l (ia|jl) t2[l,k,b,c]          Eq. (2)
  *                 (P = the 6 simultaneous permutations of (i,a),(j,b),(k,c))
  *   V_ijk[abc]  = W + t1[i,a](jb|kc) + t1[j,b](ia|kc) + t1[k,c](ia|jb)              Eqs. (6),(7)
+ *                 [+ f[i,a] t2[j,k,b,c] + f[j,b] t2[i,k,a,c] + f[k,c] t2[i,j,a,b]    Eqs. (5),(7), only when
+ *                    bqc_t_opts.f_ov is given: non-canonical reference, SURVEY.md §8(f) NEXT-3]
  *   R_ijk[abc]  = 4W[abc] + W[bca] + W[cab] - 2(W[acb] + W[cba] + W[bac])           Eq. (3)
  *   D_ijk[abc]  = eps_i + eps_j + eps_k - eps_a - eps_b - eps_c                      Eq. (3)
  *   e_ijk       = (2 - d_ij - d_jk) sum_abc R V / D            (i <= j <= k)        Eq. (4)
@@ -67,10 +69,15 @@ typedef struct bqc_t_opts {
   int max_batch;     /* triplets per W-builder launch (0 = auto from memory)                 */
   int flags;         /* BQC_T_FLAG_* below                                                   */
   int reserved;
+  const double* f_ov;/* non-canonical reference (Eqs. (5),(7); reading G15): the
+                        occupied-virtual Fock block f[i,a], [nocc][nvir], caller-owned, read-only;
+                        DEVICE memory for bqc_t_energy_ex, HOST memory for bqc_t_energy_host.
+                        V gains f[i,a] t2[j,k,b,c] + f[j,b] t2[i,k,a,c] + f[k,c] t2[i,j,a,b].
+                        NULL (default) = canonical RHF, F_ov = 0 (reading G7).               */
 } bqc_t_opts;
 
 enum {
-  BQC_T_FLAG_NO_T1 = 1,         /* drop the t1 (E[5]) term: V = W (for the E[4]-only checks)  */
+  BQC_T_FLAG_NO_T1 = 1,         /* drop the t1 (E[5]) and Fock terms: V = W (E[4]-only checks) */
   BQC_T_FLAG_PROFILE = 2        /* bracket every kernel group with CUDA events on its launching
                                    stream; read the sums with bqc_t_last_profile             */
 };
@@ -159,12 +166,13 @@ BQC_API int bqc_t_debug_slabs(int nocc, int nvir, int naux,
 
 /* Rows a2+a3: W_ijk and V_ijk of one triplet, dense [nvir][nvir][nvir] device outputs (either
    may be NULL), produced by the same slab former, W builder and V assembly as the energy path.
-   (i, j, k) need not be ordered. */
+   (i, j, k) need not be ordered.  f_ov: DEVICE [nocc][nvir] occupied-virtual Fock block or NULL
+   (see bqc_t_opts.f_ov); it enters V only. */
 BQC_API int bqc_t_debug_wv(int nocc, int nvir, int naux,
                    const double* eps_occ, const double* eps_vir,
                    const double* t1, const double* t2,
                    const double* B_oo, const double* B_ov, const double* B_vv,
-                   int i, int j, int k, double* W_dev, double* V_dev, void* stream);
+                   const double* f_ov, int i, int j, int k, double* W_dev, double* V_dev, void* stream);
 
 /* ---- building blocks exposed for measurement ------------------------------------------------ */
 

@@ -26,7 +26,7 @@ class BqcError(RuntimeError):
 class bqc_t_opts(Structure):
     _fields_ = [("occ_block", c_int), ("occ_lo", c_int), ("occ_hi", c_int),
                 ("shard_rank", c_int), ("shard_count", c_int), ("max_batch", c_int),
-                ("flags", c_int), ("reserved", c_int)]
+                ("flags", c_int), ("reserved", c_int), ("f_ov", c_void_p)]
 
 
 BQC_T_FLAG_NO_T1 = 1
@@ -75,7 +75,7 @@ def lib():
     L.bqc_t_debug_slabs.restype = c_int
     L.bqc_t_debug_slabs.argtypes = [c_int] * 3 + [dp] * 4 + [c_int, c_int] + [dp] * 3 + [c_void_p]
     L.bqc_t_debug_wv.restype = c_int
-    L.bqc_t_debug_wv.argtypes = [c_int] * 3 + [dp] * 7 + [c_int] * 3 + [dp] * 2 + [c_void_p]
+    L.bqc_t_debug_wv.argtypes = [c_int] * 3 + [dp] * 8 + [c_int] * 3 + [dp] * 2 + [c_void_p]
     L.bqc_dgemm_nt.restype = c_int
     L.bqc_dgemm_nt.argtypes = [c_int] * 3 + [dp, c_int, dp, c_int, dp, c_int, c_void_p]
     L.bqc_fp64_peak_tflops.restype = c_double
@@ -119,8 +119,16 @@ def _inputs(nocc, nvir, naux, arrays, device):
     return [_ptr(t, s, n, device) for t, s, n in zip(arrays, _shapes(nocc, nvir, naux), _NAMES)]
 
 
-def make_opts(occ_block=0, occ_lo=0, occ_hi=0, shard_rank=0, shard_count=1, max_batch=0, flags=0):
-    return bqc_t_opts(occ_block, occ_lo, occ_hi, shard_rank, shard_count, max_batch, flags, 0)
+def make_opts(occ_block=0, occ_lo=0, occ_hi=0, shard_rank=0, shard_count=1, max_batch=0, flags=0, f_ov=None):
+    """`f_ov`: optional [nocc, nvir] float64 tensor (CUDA for bqc_t_energy_ex, host for bqc_t_energy_host);
+    the returned struct keeps a reference so the pointer stays valid."""
+    o = bqc_t_opts(occ_block, occ_lo, occ_hi, shard_rank, shard_count, max_batch, flags, 0, None)
+    if f_ov is not None:
+        if f_ov.dtype != torch.float64 or not f_ov.is_contiguous() or f_ov.dim() != 2:
+            raise ValueError("f_ov must be a contiguous float64 [nocc, nvir] tensor")
+        o.f_ov = f_ov.data_ptr()
+        o._f_ov_keepalive = f_ov
+    return o
 
 
 def _optp(opts):
@@ -233,8 +241,9 @@ def bqc_t_debug_slabs(nocc, nvir, naux, t2, B_oo, B_ov, B_vv, x, y, want_I=True,
 
 
 def bqc_t_debug_wv(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, i, j, k,
-                   want_W=True, want_V=True):
+                   want_W=True, want_V=True, f_ov=None):
     p = _inputs(nocc, nvir, naux, (eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv), True)
+    p.append(_ptr(f_ov, (nocc, nvir), "f_ov", True) if f_ov is not None else None)
     dev = t2.device
     W = torch.empty((nvir, nvir, nvir), dtype=torch.float64, device=dev) if want_W else None
     V = torch.empty((nvir, nvir, nvir), dtype=torch.float64, device=dev) if want_V else None

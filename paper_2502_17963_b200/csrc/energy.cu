@@ -11,6 +11,8 @@
 // 35 KB of shared memory and 256 threads per CTA: several CTAs per SM, so the HBM reads of one orbit
 // overlap the shared-memory and FP64 work of the others.
 // Reductions are fixed-order: warp shuffle tree -> per-CTA slot -> per-triplet sum -> final sum.
+#include <type_traits>
+
 #include "kernels.cuh"
 
 namespace bqc {
@@ -46,6 +48,13 @@ struct EnergySmem {
   double epsv[3][kET];
   double red[kEThreads / 32];
 };
+// extra operands of the non-canonical Fock term (Eqs. (5),(7), reading G15):
+// V += f[i,a] t2[j,k,b,c] + f[j,b] t2[i,k,a,c] + f[k,c] t2[i,j,a,b] — same shape as the t1 (ov|ov) term
+struct FockSmem {
+  double Tt[3][6][kET * kJPitch];   // t2[y,z] tiles, indexed like Jt
+  double fs[3][3][kET];             // f_ov rows, indexed like t1s
+};
+struct NoSmem {};
 
 __device__ __forceinline__ size_t blk_off(int nb, int P, int Q, int R) {
   return (((size_t)P * nb + Q) * nb + R) * kTileElems;
@@ -53,8 +62,10 @@ __device__ __forceinline__ size_t blk_off(int nb, int P, int Q, int R) {
 
 }  // namespace
 
+template <bool kFock>
 __global__ void __launch_bounds__(kEThreads, 3) energy_kernel(const EnergyArgs a) {
   __shared__ EnergySmem sm;
+  __shared__ typename std::conditional<kFock, FockSmem, NoSmem>::type fk;
   const int tid = threadIdx.x;
   const int orbit = blockIdx.x;
   const int tb = blockIdx.y;
@@ -93,6 +104,7 @@ __global__ void __launch_bounds__(kEThreads, 3) energy_kernel(const EnergyArgs a
     const int occ = which == 0 ? tr.i : (which == 1 ? tr.j : tr.k);
     const int av = blk[pos] * kET + l;
     sm.t1s[which][pos][l] = (av < v) ? a.t1[(size_t)occ * v + av] : 0.0;
+    if constexpr (kFock) fk.fs[which][pos][l] = (av < v) ? a.f_ov[(size_t)occ * v + av] : 0.0;
   } else if (tid < 3 * 3 * kET + 3 * kET) {
     const int e = tid - 3 * 3 * kET;
     const int l = e & 7, pos = e >> 3;
@@ -111,6 +123,13 @@ __global__ void __launch_bounds__(kEThreads, 3) energy_kernel(const EnergyArgs a
       const int t = (pr & 1) ? (s == 2 ? 1 : 2) : (s == 0 ? 1 : 0);
       const int gu = blk[s] * kET + lu, gw = blk[t] * kET + lw;
       sm.Jt[m][pr][lu * kJPitch + lw] = (gu < v && gw < v) ? __ldg(Jm + (size_t)gu * v + gw) : 0.0;
+      if constexpr (kFock) {
+        // T^(0) = t2[j,k], T^(1) = t2[i,k], T^(2) = t2[i,j]
+        const int ox = (m == 0) ? tr.j : tr.i;
+        const int oy = (m == 2) ? tr.j : tr.k;
+        const double* Tm = a.t2 + ((size_t)ox * a.o + oy) * v * v;
+        fk.Tt[m][pr][lu * kJPitch + lw] = (gu < v && gw < v) ? __ldg(Tm + (size_t)gu * v + gw) : 0.0;
+      }
     }
   }
 
@@ -159,6 +178,8 @@ __global__ void __launch_bounds__(kEThreads, 3) energy_kernel(const EnergyArgs a
           const int sA = (m == 0) ? 1 : 0, sB = (m == 2) ? 1 : 2;
           const int pm = kPerm[p][m], pa = kPerm[p][sA], pb = kPerm[p][sB];
           vp = fma(sm.t1s[m][pm][l[pm]], sm.Jt[m][kPairIdx[pa][pb]][l[pa] * kJPitch + l[pb]], vp);
+          if constexpr (kFock)
+            vp = fma(fk.fs[m][pm][l[pm]], fk.Tt[m][kPairIdx[pa][pb]][l[pa] * kJPitch + l[pb]], vp);
         }
       }
       // R at the permuted point = 3 w_p + (sum of same-parity w) - 2 (sum of opposite-parity w)   (Eq. (3))
@@ -189,7 +210,10 @@ __global__ void __launch_bounds__(kEThreads, 3) energy_kernel(const EnergyArgs a
 int launch_energy(const EnergyArgs& a, cudaStream_t s) {
   if (a.ntrip <= 0) return BQC_OK;
   dim3 grid(a.norbits, a.ntrip);
-  energy_kernel<<<grid, kEThreads, 0, s>>>(a);
+  if (a.use_t1 && a.f_ov)
+    energy_kernel<true><<<grid, kEThreads, 0, s>>>(a);
+  else
+    energy_kernel<false><<<grid, kEThreads, 0, s>>>(a);
   count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
@@ -250,7 +274,10 @@ int launch_final_sum(const double* e_trip, long long n, double* out, cudaStream_
 __global__ void assemble_wv_kernel(const double* __restrict__ F, int nb, int v, const double* __restrict__ Jjk,
                                    const double* __restrict__ Jik, const double* __restrict__ Jij,
                                    const double* __restrict__ t1i, const double* __restrict__ t1j,
-                                   const double* __restrict__ t1k, double* __restrict__ W,
+                                   const double* __restrict__ t1k, const double* __restrict__ Tjk,
+                                   const double* __restrict__ Tik, const double* __restrict__ Tij,
+                                   const double* __restrict__ fi, const double* __restrict__ fj,
+                                   const double* __restrict__ fk, double* __restrict__ W,
                                    double* __restrict__ V) {
   const size_t fsz = (size_t)nb * nb * nb * kTileElems;
   const long long total = (long long)v * v * v;
@@ -264,19 +291,27 @@ __global__ void assemble_wv_kernel(const double* __restrict__ F, int nb, int v, 
     };
     const double w = at(F, a, b, c) + at(F + fsz, a, c, b) + at(F + 2 * fsz, b, c, a);
     if (W) W[e] = w;
-    if (V)
-      V[e] = w + t1i[a] * Jjk[(size_t)b * v + c] + t1j[b] * Jik[(size_t)a * v + c] +
-             t1k[c] * Jij[(size_t)a * v + b];
+    if (V) {
+      double val = w + t1i[a] * Jjk[(size_t)b * v + c] + t1j[b] * Jik[(size_t)a * v + c] +
+                   t1k[c] * Jij[(size_t)a * v + b];
+      if (fi) val += fi[a] * Tjk[(size_t)b * v + c] + fj[b] * Tik[(size_t)a * v + c] + fk[c] * Tij[(size_t)a * v + b];
+      V[e] = val;
+    }
   }
 }
 
 int launch_assemble_wv(const double* F, int nbv, int v, const double* J, int nw, int pi, int pj, int pk,
-                       const double* t1i, const double* t1j, const double* t1k, double* W, double* V,
-                       cudaStream_t s) {
+                       const double* t1i, const double* t1j, const double* t1k, const double* t2, int o, int i,
+                       int j, int k, const double* f_ov, double* W, double* V, cudaStream_t s) {
   const size_t v2 = (size_t)v * v;
+  const bool fock = f_ov != nullptr;
   assemble_wv_kernel<<<1024, 256, 0, s>>>(F, nbv, v, J + ((size_t)pj * nw + pk) * v2,
                                           J + ((size_t)pi * nw + pk) * v2, J + ((size_t)pi * nw + pj) * v2,
-                                          t1i, t1j, t1k, W, V);
+                                          t1i, t1j, t1k, fock ? t2 + ((size_t)j * o + k) * v2 : nullptr,
+                                          fock ? t2 + ((size_t)i * o + k) * v2 : nullptr,
+                                          fock ? t2 + ((size_t)i * o + j) * v2 : nullptr,
+                                          fock ? f_ov + (size_t)i * v : nullptr, fock ? f_ov + (size_t)j * v : nullptr,
+                                          fock ? f_ov + (size_t)k * v : nullptr, W, V);
   count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;

@@ -33,8 +33,10 @@ struct EnergyArgs {
   const double* t1;         // [o][v]
   const double* eps_occ;    // [o]
   const double* eps_vir;    // [v]
+  const double* t2;         // [o][o][v][v]   (Fock term only)
+  const double* f_ov;       // [o][v] occupied-virtual Fock block, or NULL (canonical reference)
   double* partial;          // [ntrip][norbits]
-  int ntrip, norbits, nbv, v, nw, use_t1;
+  int ntrip, norbits, nbv, v, nw, use_t1, o;
 };
 int launch_energy(const EnergyArgs& a, cudaStream_t s);
 
@@ -46,8 +48,8 @@ int launch_final_sum(const double* e_trip, long long n, double* out, cudaStream_
 
 // dense W / V [v][v][v] of one triplet from its three blocked F arrays (debug / parity of rows a2, a3)
 int launch_assemble_wv(const double* F, int nbv, int v, const double* J, int nw, int pi, int pj, int pk,
-                       const double* t1i, const double* t1j, const double* t1k, double* W, double* V,
-                       cudaStream_t s);
+                       const double* t1i, const double* t1j, const double* t1k, const double* t2, int o, int i,
+                       int j, int k, const double* f_ov, double* W, double* V, cudaStream_t s);
 
 // strided 3-D copy out[a][b][c] = in[a*sa + b*sb + c*sc], used to unpad debug slabs
 int launch_copy3(const double* in, long long sa, long long sb, long long sc, double* out, int na, int nb,

@@ -215,6 +215,7 @@ int check_device() {
 
 struct Inputs {
   const double *eps_occ, *eps_vir, *t1, *t2, *B_oo, *B_ov, *B_vv;
+  const double* f_ov = nullptr;   // optional occupied-virtual Fock block (bqc_t_opts.f_ov)
 };
 
 // ------------------------------------------------------------------ run context
@@ -629,6 +630,7 @@ int Pipeline::compute(const Action& a) {
   e.F = c.F(); e.trips = c.trips_dev() + a.trip0; e.orbits = c.orbits_dev();
   e.J = c.J(); e.t1 = c.in.t1; e.eps_occ = c.in.eps_occ; e.eps_vir = c.in.eps_vir;
   e.partial = c.partial();
+  e.t2 = c.in.t2; e.f_ov = c.in.f_ov; e.o = P.o;
   e.ntrip = (int)a.ntrip; e.norbits = P.norbits; e.nbv = P.nbv; e.v = v; e.nw = P.na; e.use_t1 = P.use_t1;
   BQC_TRY(launch_energy(e, s));
   BQC_TRY(launch_reduce_triplets(c.partial(), c.trips_dev() + a.trip0, (int)a.ntrip, P.norbits, c.etrip(), s));
@@ -698,6 +700,7 @@ int t_energy_impl(int o, int v, int X, const Inputs& in, const bqc_t_opts* opts,
     return BQC_ERR_NULL_POINTER;
   }
   BQC_TRY(validate_inputs(o, v, X, in));
+  if (in.f_ov) BQC_TRY(check_device_ptr(in.f_ov, "opts->f_ov"));
   if (e_triplet_dev) BQC_TRY(check_device_ptr(e_triplet_dev, "e_triplet_dev"));
   int lo, hi;
   BQC_TRY(resolve_window(o, opts, &lo, &hi));
@@ -855,7 +858,7 @@ int bqc_t_energy_ex(int nocc, int nvir, int naux, const double* eps_occ, const d
                     const double* t1, const double* t2, const double* B_oo, const double* B_ov,
                     const double* B_vv, const bqc_t_opts* opts, void* workspace, size_t workspace_bytes,
                     double* e_total_host, double* e_triplet_dev, void* stream) {
-  Inputs in = {eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv};
+  Inputs in = {eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, opts ? opts->f_ov : nullptr};
   return t_energy_impl(nocc, nvir, naux, in, opts, workspace, workspace_bytes, e_total_host, e_triplet_dev,
                        static_cast<cudaStream_t>(stream));
 }
@@ -876,11 +879,13 @@ int bqc_t_energy_host(int nocc, int nvir, int naux, const double* eps_occ, const
   clear_error();
   cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
   BQC_TRY(check_sizes(nocc, nvir, naux));
-  const void* ptrs[7] = {eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv};
-  const char* names[7] = {"eps_occ", "eps_vir", "t1", "t2", "B_oo", "B_ov", "B_vv"};
+  const bool fock = opts && opts->f_ov;
+  const int nin = fock ? 8 : 7;
+  const void* ptrs[8] = {eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, fock ? opts->f_ov : nullptr};
+  const char* names[8] = {"eps_occ", "eps_vir", "t1", "t2", "B_oo", "B_ov", "B_vv", "opts->f_ov"};
   const size_t o = nocc, v = nvir, X = naux;
-  const size_t elems[7] = {o, v, o * v, o * o * v * v, X * o * o, X * o * v, X * v * v};
-  for (int n = 0; n < 7; ++n)
+  const size_t elems[8] = {o, v, o * v, o * o * v * v, X * o * o, X * o * v, X * v * v, o * v};
+  for (int n = 0; n < nin; ++n)
     if (!ptrs[n]) {
       set_error(BQC_ERR_NULL_POINTER, "%s is NULL", names[n]);
       return BQC_ERR_NULL_POINTER;
@@ -889,8 +894,8 @@ int bqc_t_energy_host(int nocc, int nvir, int naux, const double* eps_occ, const
     set_error(BQC_ERR_NULL_POINTER, "e_total_host is NULL");
     return BQC_ERR_NULL_POINTER;
   }
-  size_t total = 0, offs[7];
-  for (int n = 0; n < 7; ++n) { offs[n] = total; total += round_up(elems[n] * 8, 256); }
+  size_t total = 0, offs[8];
+  for (int n = 0; n < nin; ++n) { offs[n] = total; total += round_up(elems[n] * 8, 256); }
   const size_t ntrip = num_triplets(nocc);
   const size_t off_trip = total;
   total += round_up(ntrip * 8, 256);
@@ -905,7 +910,7 @@ int bqc_t_energy_host(int nocc, int nvir, int naux, const double* eps_occ, const
   }
   int rc = BQC_OK;
   size_t h2d = 0;
-  for (int n = 0; n < 7 && rc == BQC_OK; ++n) {
+  for (int n = 0; n < nin && rc == BQC_OK; ++n) {
     cudaError_t e = cudaMemcpyAsync(dev + offs[n], ptrs[n], elems[n] * 8, cudaMemcpyHostToDevice, stream);
     if (e != cudaSuccess) {
       set_error(BQC_ERR_CUDA, "H2D copy of %s failed: %s", names[n], cudaGetErrorString(e));
@@ -915,7 +920,11 @@ int bqc_t_energy_host(int nocc, int nvir, int naux, const double* eps_occ, const
   }
   if (rc == BQC_OK) {
     auto D = [&](int n) { return reinterpret_cast<const double*>(dev + offs[n]); };
-    rc = bqc_t_energy_ex(nocc, nvir, naux, D(0), D(1), D(2), D(3), D(4), D(5), D(6), opts, nullptr, 0,
+    bqc_t_opts dopts;
+    memset(&dopts, 0, sizeof(dopts));
+    if (opts) dopts = *opts;
+    dopts.f_ov = fock ? D(7) : nullptr;   // the device copy replaces the caller's host pointer
+    rc = bqc_t_energy_ex(nocc, nvir, naux, D(0), D(1), D(2), D(3), D(4), D(5), D(6), &dopts, nullptr, 0,
                          e_total_host, e_triplet_host ? reinterpret_cast<double*>(dev + off_trip) : nullptr,
                          stream);
   }
@@ -992,11 +1001,13 @@ int bqc_t_debug_slabs(int nocc, int nvir, int naux, const double* t2, const doub
 
 int bqc_t_debug_wv(int nocc, int nvir, int naux, const double* eps_occ, const double* eps_vir,
                    const double* t1, const double* t2, const double* B_oo, const double* B_ov,
-                   const double* B_vv, int i, int j, int k, double* W_dev, double* V_dev, void* stream_v) {
+                   const double* B_vv, const double* f_ov, int i, int j, int k, double* W_dev, double* V_dev,
+                   void* stream_v) {
   clear_error();
   cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
-  Inputs in = {eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv};
+  Inputs in = {eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, f_ov};
   BQC_TRY(validate_inputs(nocc, nvir, naux, in));
+  if (f_ov) BQC_TRY(check_device_ptr(f_ov, "f_ov"));
   if (i < 0 || j < 0 || k < 0 || i >= nocc || j >= nocc || k >= nocc) {
     set_error(BQC_ERR_INVALID_SIZE, "triplet (%d,%d,%d) outside [0,%d)", i, j, k, nocc);
     return BQC_ERR_INVALID_SIZE;
@@ -1053,7 +1064,8 @@ int bqc_t_debug_wv(int nocc, int nvir, int naux, const double* eps_occ, const do
   prm.C = c.F();
   BQC_TRY(launch_gemm_nt(c.f_nf, c.tm_slab, c.tm_slabT, c.tm_btil, prm, stream));
   BQC_TRY(launch_assemble_wv(c.F(), P.nbv, nvir, c.J(), P.na, pi, pj, pk, t1 + (size_t)i * nvir,
-                             t1 + (size_t)j * nvir, t1 + (size_t)k * nvir, W_dev, V_dev, stream));
+                             t1 + (size_t)j * nvir, t1 + (size_t)k * nvir, t2, nocc, i, j, k, f_ov, W_dev, V_dev,
+                             stream));
   BQC_CUDA_OK(cudaStreamSynchronize(stream));
   BQC_CUDA_OK(cudaStreamSynchronize(c.s_form));
   return BQC_OK;

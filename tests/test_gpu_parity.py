@@ -252,3 +252,38 @@ def test_errors_are_reported():
     import math
     assert math.isnan(L.bqc_t_energy(0, v, x, *ptrs, None))
     assert call() == 0                                           # and the library still works
+
+
+# ------------------------------------------------------------------ NEXT-3: occupied-virtual Fock block
+@pytest.mark.parametrize("case", ["o3v16", "config1", "ragged"])
+def test_fock_term_energy_and_v(case):
+    """PAPER.md:298-303 Eqs. (5),(7) (reading G15): V += f[i,a] t2[j,k,b,c] + f[j,b] t2[i,k,a,c] + f[k,c] t2[i,j,a,b]."""
+    import copy
+    inp = {"o3v16": lambda: make_inputs(3, 16, 10, seed=41, t1_std=0.05, f_std=0.1),
+           "config1": lambda: make_config(1, t1_std=0.05, f_std=0.05),
+           "ragged": lambda: make_inputs(4, 35, 41, seed=42, t1_std=0.05, f_std=0.1)}[case]()
+    d = to_device(inp)
+    f_dev = torch.from_numpy(inp.f_ov).cuda()
+    e_ref, trip_ref = orc.t_energy(inp, return_triplets=True)
+    canon = copy.copy(inp)
+    canon.f_ov = None
+    e_canon = orc.t_energy(canon)
+    assert abs(e_ref - e_canon) > 1e-6 * abs(e_ref)          # the term carries weight in this input
+    et = torch.empty(bqc.bqc_t_num_triplets(inp.nocc), dtype=torch.float64, device="cuda")
+    e = bqc.bqc_t_energy_ex(*dims(inp), *d, opts=bqc.make_opts(f_ov=f_dev), e_triplet=et)
+    assert abs(e - e_ref) <= e_tol(e_ref)
+    n = len(trip_ref)
+    assert np.all(np.abs(et.cpu().numpy() - trip_ref) <= 1e-10 * np.abs(trip_ref) + 1e-12 * abs(e_ref) / n + 1e-300)
+    # without f_ov the canonical value comes back; the host entry point copies f_ov itself
+    assert abs(bqc.bqc_t_energy_ex(*dims(inp), *d) - e_canon) <= e_tol(e_canon)
+    host = [torch.from_numpy(np.ascontiguousarray(a)) for a in inp.arrays()]
+    e_host, h2d, _ = bqc.bqc_t_energy_host(*dims(inp), *host, opts=bqc.make_opts(f_ov=torch.from_numpy(inp.f_ov)))
+    assert e_host == e
+    assert h2d == inp.nbytes() + inp.f_ov.nbytes
+    # V element by element
+    o = inp.nocc
+    for (i, j, k) in [(0, 1, 2), (0, 0, o - 1), (2, 0, 1)]:
+        W, V = bqc.bqc_t_debug_wv(*dims(inp), *d, i, j, k, f_ov=f_dev)
+        Wr = orc.w_triplet(inp, i, j, k)
+        _close(W, Wr)
+        _close(V, orc.v_triplet(inp, i, j, k, Wr))
