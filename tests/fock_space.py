@@ -34,8 +34,8 @@ def _jw_annihilators(nso):
     return ops
 
 
-def first_principles_t(inp, with_fock=False):
-    """Return (E4, E5) — or (E4, E5, EF) with `with_fock` — for a TInputs; feasible for o+v <= 7."""
+def _model(inp):
+    """(E_pq, apply_WN, |HF>, eps, nso) of the model Hamiltonian H0 = sum_p eps_p E_pp, H = H0 + W_N."""
     o, v = inp.nocc, inp.nvir
     n = o + v
     nso = 2 * n
@@ -76,6 +76,48 @@ def first_principles_t(inp, with_fock=False):
     idx0 = sum(1 << (nso - 1 - s) for s in range(2 * o))
     hf = np.zeros(dim)
     hf[idx0] = 1.0
+    eps = np.concatenate([inp.eps_occ, inp.eps_vir])
+    return E, apply_WN, hf, eps, nso
+
+
+def _resolvent(o, eps, nso, rank):
+    """diag(1/D) on the determinants with `rank` holes and `rank` particles, D = sum eps_holes - sum eps_particles."""
+    dim = 1 << nso
+    r = np.zeros(dim)
+    for d in range(dim):
+        holes, parts, D = 0, 0, 0.0
+        for s in range(nso):
+            occd = (d >> (nso - 1 - s)) & 1
+            p = s // 2
+            if p < o and not occd:
+                holes += 1
+                D += eps[p]
+            elif p >= o and occd:
+                parts += 1
+                D -= eps[p]
+        if holes == rank and parts == rank:
+            r[d] = 1.0 / D
+    return r
+
+
+def first_principles_mp2(inp):
+    """Second-order Rayleigh-Schroedinger energy E2 = <0| W_N R W_N |0> of the model Hamiltonian, R the
+    resolvent of H0 on singly and doubly excited determinants.  Uses no index formula of PAPER.md Eq. (1).
+    Returns (E2_doubles, E2_singles); the singles part vanishes because W_N is normal ordered w.r.t. the
+    HF mean field (Brillouin).  Feasible for o+v <= 7."""
+    o = inp.nocc
+    E, apply_WN, hf, eps, nso = _model(inp)
+    psi = apply_WN(hf)
+    r2 = _resolvent(o, eps, nso, 2)
+    r1 = _resolvent(o, eps, nso, 1)
+    return float(psi @ (r2 * psi)), float(psi @ (r1 * psi))
+
+
+def first_principles_t(inp, with_fock=False):
+    """Return (E4, E5) — or (E4, E5, EF) with `with_fock` — for a TInputs; feasible for o+v <= 7."""
+    o, v = inp.nocc, inp.nvir
+    E, apply_WN, hf, eps, nso = _model(inp)
+    dim = 1 << nso
 
     t1v = np.zeros(dim)
     for i in range(o):
@@ -93,21 +135,7 @@ def first_principles_t(inp, with_fock=False):
     phi = apply_WN(t1v)
 
     # R3 on determinants
-    eps = np.concatenate([inp.eps_occ, inp.eps_vir])
-    r3 = np.zeros(dim)
-    for d in range(dim):
-        holes, parts, D = 0, 0, 0.0
-        for s in range(nso):
-            occd = (d >> (nso - 1 - s)) & 1
-            p = s // 2
-            if p < o and not occd:
-                holes += 1
-                D += eps[p]
-            elif p >= o and occd:
-                parts += 1
-                D -= eps[p]
-        if holes == 3 and parts == 3:
-            r3[d] = 1.0 / D
+    r3 = _resolvent(o, eps, nso, 3)
     e4, e5 = float(psi @ (r3 * psi)), float(phi @ (r3 * psi))
     if not with_fock:
         return e4, e5
