@@ -50,6 +50,8 @@ def parse():
     ap.add_argument("--peak-seconds", type=float, default=2.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-triplets", type=int, default=3, help="triplets the oracle evaluates (cpu_baseline)")
+    ap.add_argument("--path", default="t", choices=["t", "mp2"],
+                    help="t: the (T) energy (the headline); mp2: the DF-MP2 energy of PAPER.md Eq. (1) (SURVEY NEXT-4)")
     return ap.parse_args()
 
 
@@ -161,6 +163,75 @@ def run_reference(args, rank, world):
     print(json.dumps(out), flush=True)
 
 
+# ----------------------------------------------------------------------------- DF-MP2
+def run_mp2(args):
+    """One step = one whole E_MP2 evaluation of the config (single GPU).  value = algorithmic (ov|ov) flops
+    o(o+1)/2 * 2 v^2 X / device time."""
+    import paper_2502_17963_b200 as bqc
+    from bqc_inputs import CONFIGS, make_config
+    torch.cuda.set_device(0)
+    c = CONFIGS[args.config]
+    o, v, X = c["nocc"], c["nvir"], c["naux"]
+    inp = make_config(args.config)
+    host = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (inp.eps_occ, inp.eps_vir, inp.B_ov)]
+    dev = [t.cuda() for t in host]
+    opts = bqc.make_mp2_opts(occ_block=args.occ_block, flags=bqc.BQC_T_FLAG_PROFILE)
+    peak = bqc.bqc_fp64_peak_tflops(0, args.peak_seconds)
+    e_pair = torch.zeros((o, o), dtype=torch.float64, device="cuda")
+    for _ in range(args.warmup):
+        e_val = bqc.bqc_mp2_energy_ex(o, v, X, *dev, opts=opts, e_pair=e_pair)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches = 0
+    ev0.record()
+    for _ in range(args.steps):
+        e_val = bqc.bqc_mp2_energy_ex(o, v, X, *dev, opts=opts, e_pair=e_pair)
+        prof = bqc.bqc_mp2_last_profile()
+        launches += int(prof["kernel_launches"])
+    ev1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1) / max(args.steps, 1)
+    flops = bqc.bqc_mp2_flops(o, v, X)
+    t0 = time.perf_counter()
+    for _ in range(max(args.e2e_steps, 1)):
+        e_host, h2d, d2h = bqc.bqc_mp2_energy_host(o, v, X, *host)
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / max(args.e2e_steps, 1)
+    assert e_host == e_val
+    gemm_tf = flops / (prof["gemm_ms"] * 1e-3) * 1e-12
+    out = {"metric": "DF-MP2 FP64 TFLOP/s ((ov|ov) algorithmic flops / whole-path time)", "value": flops / (ms * 1e-3) * 1e-12,
+           "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": f"DF-MP2 energy, config{args.config} nocc={o} nvir={v} naux={X}, all {o * (o + 1) // 2} pairs i<=j",
+                      "occ_block": bqc.bqc_mp2_plan_occ_block(o, v, X, opts)},
+           "e_mp2_hartree": e_val, "fp64_tensor_peak_tflops_measured": peak,
+           "kernel_ms_per_step": {"ovov_gemm": prof["gemm_ms"], "pair_energy": prof["energy_ms"], "call_total": prof["total_ms"]},
+           "roofline": {"bound": "tensor", "kernel": "gemm_nt_kernel ((ov|ov) former)", "achieved": gemm_tf, "peak": peak,
+                        "unit": UNIT, "frac": gemm_tf / peak, "traffic": None},
+           "clocks": clocks,
+           "e2e": {"value": flops / (e2e_ms * 1e-3) * 1e-12, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                   "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms},
+           "gpu_launches": launches}
+    if not args.no_cpu_baseline:
+        from oracle import mp2_oracle as orc_mp2        # bench.py's cpu_baseline leg only
+        npairs = min(o * o, 64)
+        t0 = time.perf_counter()
+        worst = 0.0
+        e_gpu = e_pair.cpu().numpy()
+        for n in range(npairs):
+            i, j = n % o, (n * 7) % o
+            ref = orc_mp2.pair_energy(inp, i, j)
+            worst = max(worst, abs(e_gpu[i, j] - ref) / (1e-10 * abs(ref) + 1e-12 * abs(e_val) / (o * o)))
+        dt = time.perf_counter() - t0
+        out["cpu_baseline"] = {"value": npairs * 2.0 * v * v * X / dt * 1e-12, "unit": UNIT, "cores": cpu_threads(),
+                               "kind": "oracle", "sample": f"{npairs} pairs of the workload in {dt:.2f} s, NumPy oracle as it stands",
+                               "gpu_vs_oracle_worst_err_over_tol": worst}
+        assert worst <= 1.0
+    print(json.dumps(out), flush=True)
+
+
 # ----------------------------------------------------------------------------- our arm
 def main():
     args = parse()
@@ -178,6 +249,10 @@ def main():
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the CUDA library is the only implementation")
+    if args.path == "mp2":
+        if rank == 0:
+            run_mp2(args)
+        return
     torch.cuda.set_device(local_rank)
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")

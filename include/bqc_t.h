@@ -174,6 +174,53 @@ BQC_API int bqc_t_debug_wv(int nocc, int nvir, int naux,
                    const double* B_oo, const double* B_ov, const double* B_vv,
                    const double* f_ov, int i, int j, int k, double* W_dev, double* V_dev, void* stream);
 
+/* ---- closed-shell DF-MP2 energy ------------------------------------ */
+
+/* PAPER.md:252-258 (§2.3, Eq. (1)), unrestricted closed-shell sum (reading M1 in DESIGN.md):
+     J_ij[a,b] = (ia|jb) = sum_Q B_ov[Q,i,a] B_ov[Q,j,b]                       (exact DF)
+     e_ij      = sum_ab J_ij[a,b] (2 J_ij[a,b] - J_ij[b,a]) / (eps_i + eps_j - eps_a - eps_b)
+     E_MP2     = sum_{i,j} e_ij = sum_{i<=j} (2 - d_ij) e_ij                   (e_ij = e_ji)
+   The (ov|ov) integrals are formed block by block with the library's TMA + DMMA tile GEMM and never
+   stored whole; the denominator is evaluated in registers from the orbital energies.
+   Options, zero-initialise for defaults. */
+typedef struct bqc_mp2_opts {
+  int occ_block;     /* occupied orbitals i per (ov|ov) block (0 = auto: block buffer <= 2 GiB)     */
+  int shard_rank;    /* multi-GPU sharding: this call evaluates the occupied blocks whose number     */
+  int shard_count;   /*   % shard_count == shard_rank (all pairs i <= j of those rows i).  0 -> 1.  */
+  int flags;         /* BQC_T_FLAG_PROFILE: time the kernel groups, read with bqc_mp2_last_profile  */
+} bqc_mp2_opts;
+
+/* E_MP2 in Hartree; NaN on error.  DEVICE pointers: eps_occ [nocc], eps_vir [nvir],
+   B_ov [naux][nocc][nvir].  Device scratch is allocated internally and freed before return.
+   Error behaviour as bqc_t_energy; BQC_ERR_DENOMINATOR if 2*max(eps_occ) - 2*min(eps_vir) >= 0. */
+BQC_API double bqc_mp2_energy(int nocc, int nvir, int naux, const double* eps_occ, const double* eps_vir,
+                      const double* B_ov, void* stream);
+
+/* Same with options and per-pair output.
+     e_total_host  HOST pointer; receives sum_{i<=j, i in this shard's blocks} (2 - d_ij) e_ij.
+     e_pair_dev    DEVICE pointer [nocc][nocc] or NULL; receives the unweighted e_ij at [i][j] AND [j][i]
+                   for every pair this call evaluated, 0 elsewhere.
+   Returns BQC_OK or an error code. */
+BQC_API int bqc_mp2_energy_ex(int nocc, int nvir, int naux, const double* eps_occ, const double* eps_vir,
+                      const double* B_ov, const bqc_mp2_opts* opts, double* e_total_host,
+                      double* e_pair_dev, void* stream);
+
+/* End-to-end form: HOST pointers in, H2D of the three inputs and D2H of the scalar (and of the
+   [nocc][nocc] pair matrix when e_pair_host != NULL) inside the call. */
+BQC_API int bqc_mp2_energy_host(int nocc, int nvir, int naux, const double* eps_occ, const double* eps_vir,
+                        const double* B_ov, const bqc_mp2_opts* opts, double* e_total_host,
+                        double* e_pair_host, size_t* h2d_bytes, size_t* d2h_bytes, void* stream);
+
+/* Algorithmic FP64 flop count of the (ov|ov) contraction over the pairs i <= j:
+   o(o+1)/2 * 2 v^2 X (the energy reduction, ~8 flops per element, is not counted). */
+BQC_API double bqc_mp2_flops(int nocc, int nvir, int naux);
+/* Occupied block size bqc_mp2_energy_ex will use (resolves opts->occ_block == 0); -1 on bad sizes. */
+BQC_API int bqc_mp2_plan_occ_block(int nocc, int nvir, int naux, const bqc_mp2_opts* opts);
+/* Timing of this thread's last profiled bqc_mp2_energy_ex call (CUDA events on the launch stream):
+     [0] (ov|ov) tile-GEMM ms  [1] its launches  [2] pair-energy + reduction kernel ms  [3] their launches
+     [4] whole call ms         [5] library kernels launched.   Returns the number of values written. */
+BQC_API int bqc_mp2_last_profile(double* out, int n);
+
 /* ---- building blocks exposed for measurement ------------------------------------------------ */
 
 /* C[M][N] (ldc) = A[M][K] (lda) * B[N][K]^T (ldb), FP64, device pointers, the library's TMA +

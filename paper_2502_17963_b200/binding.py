@@ -29,6 +29,10 @@ class bqc_t_opts(Structure):
                 ("flags", c_int), ("reserved", c_int), ("f_ov", c_void_p)]
 
 
+class bqc_mp2_opts(Structure):
+    _fields_ = [("occ_block", c_int), ("shard_rank", c_int), ("shard_count", c_int), ("flags", c_int)]
+
+
 BQC_T_FLAG_NO_T1 = 1
 BQC_T_FLAG_PROFILE = 2
 
@@ -80,6 +84,19 @@ def lib():
     L.bqc_dgemm_nt.argtypes = [c_int] * 3 + [dp, c_int, dp, c_int, dp, c_int, c_void_p]
     L.bqc_fp64_peak_tflops.restype = c_double
     L.bqc_fp64_peak_tflops.argtypes = [c_int, c_double, c_void_p]
+    L.bqc_mp2_energy.restype = c_double
+    L.bqc_mp2_energy.argtypes = [c_int] * 3 + [dp] * 3 + [c_void_p]
+    L.bqc_mp2_energy_ex.restype = c_int
+    L.bqc_mp2_energy_ex.argtypes = [c_int] * 3 + [dp] * 3 + [POINTER(bqc_mp2_opts), POINTER(c_double), dp, c_void_p]
+    L.bqc_mp2_energy_host.restype = c_int
+    L.bqc_mp2_energy_host.argtypes = [c_int] * 3 + [dp] * 3 + [POINTER(bqc_mp2_opts), POINTER(c_double), dp,
+                                                             POINTER(c_size_t), POINTER(c_size_t), c_void_p]
+    L.bqc_mp2_flops.restype = c_double
+    L.bqc_mp2_flops.argtypes = [c_int] * 3
+    L.bqc_mp2_plan_occ_block.restype = c_int
+    L.bqc_mp2_plan_occ_block.argtypes = [c_int] * 3 + [POINTER(bqc_mp2_opts)]
+    L.bqc_mp2_last_profile.restype = c_int
+    L.bqc_mp2_last_profile.argtypes = [POINTER(c_double), c_int]
     _lib = L
     return L
 
@@ -225,6 +242,60 @@ def bqc_t_energy_host(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_
     _check(lib().bqc_t_energy_host(nocc, nvir, naux, *p, _optp(opts), byref(e), et, byref(h2d),
                                    byref(d2h), _stream()))
     return e.value, h2d.value, d2h.value
+
+
+# ---------------------------------------------------------------- DF-MP2 energy (Eq. (1))
+def make_mp2_opts(occ_block=0, shard_rank=0, shard_count=1, flags=0):
+    return bqc_mp2_opts(occ_block, shard_rank, shard_count, flags)
+
+
+def _mp2_inputs(nocc, nvir, naux, eps_occ, eps_vir, B_ov, device):
+    return [_ptr(eps_occ, (nocc,), "eps_occ", device), _ptr(eps_vir, (nvir,), "eps_vir", device),
+            _ptr(B_ov, (naux, nocc, nvir), "B_ov", device)]
+
+
+def bqc_mp2_energy(nocc, nvir, naux, eps_occ, eps_vir, B_ov):
+    """E_MP2 [Hartree] from device tensors, on torch's current CUDA stream."""
+    p = _mp2_inputs(nocc, nvir, naux, eps_occ, eps_vir, B_ov, True)
+    e = lib().bqc_mp2_energy(nocc, nvir, naux, *p, _stream())
+    if e != e:
+        _check(lib().bqc_last_error() or 6)
+    return e
+
+
+def bqc_mp2_energy_ex(nocc, nvir, naux, eps_occ, eps_vir, B_ov, opts=None, e_pair=None):
+    """Returns the weighted pair sum of this shard; `e_pair`: optional float64 CUDA [nocc, nocc] filled with e_ij."""
+    p = _mp2_inputs(nocc, nvir, naux, eps_occ, eps_vir, B_ov, True)
+    ep = _ptr(e_pair, (nocc, nocc), "e_pair", True) if e_pair is not None else None
+    e = c_double(0.0)
+    _check(lib().bqc_mp2_energy_ex(nocc, nvir, naux, *p, _optp(opts), byref(e), ep, _stream()))
+    return e.value
+
+
+def bqc_mp2_energy_host(nocc, nvir, naux, eps_occ, eps_vir, B_ov, opts=None, e_pair=None):
+    """End-to-end call with HOST tensors.  Returns (E, h2d_bytes, d2h_bytes)."""
+    p = _mp2_inputs(nocc, nvir, naux, eps_occ, eps_vir, B_ov, False)
+    ep = _ptr(e_pair, (nocc, nocc), "e_pair", False) if e_pair is not None else None
+    e = c_double(0.0)
+    h2d, d2h = c_size_t(0), c_size_t(0)
+    _check(lib().bqc_mp2_energy_host(nocc, nvir, naux, *p, _optp(opts), byref(e), ep, byref(h2d), byref(d2h),
+                                     _stream()))
+    return e.value, h2d.value, d2h.value
+
+
+def bqc_mp2_flops(nocc, nvir, naux):
+    return lib().bqc_mp2_flops(nocc, nvir, naux)
+
+
+def bqc_mp2_plan_occ_block(nocc, nvir, naux, opts=None):
+    return lib().bqc_mp2_plan_occ_block(nocc, nvir, naux, _optp(opts))
+
+
+def bqc_mp2_last_profile():
+    buf = (c_double * 6)()
+    n = lib().bqc_mp2_last_profile(buf, 6)
+    keys = ["gemm_ms", "gemm_launches", "energy_ms", "energy_launches", "total_ms", "kernel_launches"]
+    return {k: buf[i] for i, k in enumerate(keys[:n])}
 
 
 # ---------------------------------------------------------------- single steps (parity tests)

@@ -17,6 +17,11 @@ void clear_error();
 // number of kernels this thread launched (every launch_* helper counts its kernels)
 void count_launch(int n = 1);
 
+// argument checks common to every entry point (t_energy.cu); each sets the error state on failure
+int check_sizes(int nocc, int nvir, int naux);
+int check_device_ptr(const void* p, const char* name);
+int check_device();
+
 #define BQC_CUDA_OK(expr)                                                                   \
   do {                                                                                      \
     cudaError_t _e = (expr);                                                                \

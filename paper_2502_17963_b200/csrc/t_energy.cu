@@ -165,7 +165,9 @@ int make_plan(Plan& P, int o, int v, int X, const std::vector<int>& act, const b
   return BQC_OK;
 }
 
-// ------------------------------------------------------------------ argument checks
+}  // namespace
+
+// ------------------------------------------------------------------ argument checks (shared with mp2.cu)
 int check_sizes(int o, int v, int X) {
   if (o <= 0 || v <= 0 || X <= 0) {
     set_error(BQC_ERR_INVALID_SIZE, "nocc=%d nvir=%d naux=%d must all be > 0", o, v, X);
@@ -212,6 +214,8 @@ int check_device() {
   }
   return BQC_OK;
 }
+
+namespace {
 
 struct Inputs {
   const double *eps_occ, *eps_vir, *t1, *t2, *B_oo, *B_ov, *B_vv;
