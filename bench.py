@@ -233,6 +233,11 @@ def run_mp2(args):
 
 
 # ----------------------------------------------------------------------------- our arm
+# bytes per W-builder launch (4 triplets) from the one `ncu --set full` capture named in profiles/README.md:
+# 13.94 GB read + 5.24 GB written at config 5 (algorithmic: 5.27 GB of F writes + L2-shared operand reads)
+NCU_TRAFFIC_W_BUILDER = {5: 13.939768e9 + 5.243941e9}
+
+
 def main():
     args = parse()
     rank = int(os.environ.get("RANK", "0"))
@@ -376,7 +381,10 @@ def main():
                                         "mma.sync m8n8k4 loop on all SMs); MEASURED_PEAKS.json has no FP64 entry",
                          "launches": int(prof["gemm_launches"]),
                          "flops_per_launch": flops_rank / max(prof["gemm_launches"], 1),
-                         "traffic": None},
+                         "traffic": NCU_TRAFFIC_W_BUILDER.get(args.config),
+                         "traffic_source": "ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch "
+                                           "(profiles/r1b_gemm_nt_full.txt)" if args.config in NCU_TRAFFIC_W_BUILDER
+                                           else None},
             "clocks": clocks,
             "e2e": {"value": (flops_total / (e2e_ms_max * 1e-3) * 1e-12) if e2e_ms_max else None, "unit": UNIT,
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
