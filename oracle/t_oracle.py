@@ -30,6 +30,12 @@ vanishes for canonical RHF (G7); when the input carries an occupied-virtual
 Fock block ``f_ov`` V gains
 f[i,a] t2[j,k,b,c] + f[j,b] t2[i,k,a,c] + f[k,c] t2[i,j,a,b]  (reading G15).
 
+The paper's own loop order ("abc-driven") is
+written out as well — ``w_virtual_triple`` / ``v_virtual_triple`` /
+``e_virtual_triple`` / ``t_energy_abc``: one virtual triple a<=b<=c at a time, all
+o^3 occupied triples inside, E = 2 sum_{a<=b<=c} (1/alpha) sum_ijk [r3_ijk(W)/D] V
+with alpha = 1/2/6 (reading G3).  Pinned by ``tests/test_abc_oracle_pins.py``.
+
 Arithmetic is FP64 NumPy.  ``numpy.einsum`` / ``@`` serve as the library
 contraction primitive of each step; there is no blocking, fusion or reordering
 beyond the equations above.  Every function is pinned by ``tests/`` (``-m "not
@@ -165,6 +171,71 @@ def t_energy(inp, with_t1=True, return_triplets=False, cache_slabs=True):
         e[n] = e_triplet(inp, i, j, k, slabs, with_t1)
     total = float(np.sum(e.astype(np.longdouble)))
     return (total, e) if return_triplets else total
+
+
+# --------------------------------------------------------------------------
+# The paper's abc-driven loop (SURVEY.md §8(c) "Passages followed",
+# §8(f) NEXT-2): one virtual triple a,b,c at a time, o^3 tensors inside
+#     E = 2 sum_{a<=b<=c} (1/alpha) sum_ijk [r3_ijk(W) / D] V,
+# alpha = 1 / 2 / 6 for three distinct / exactly two equal / three equal virtuals
+# (reading G3), r3 the 4/1/1/-2/-2/-2 pattern of Eq. (3) applied to ijk.
+# --------------------------------------------------------------------------
+def w_virtual_triple(inp, a, b, c):
+    """W^{abc}[i,j,k] of Eq. (2) for one virtual triple and all occupied i,j,k."""
+    vir = (a, b, c)
+    o = inp.nocc
+    W = np.zeros((o, o, o))
+    for perm in _PERMS:
+        u1, u2, u3 = vir[perm[0]], vir[perm[1]], vir[perm[2]]
+        # particle: sum_d (x1 u1|u2 d) t2[x3,x2,u3,d]
+        ovvv = np.einsum("Qx,Qd->xd", inp.B_ov[:, :, u1], inp.B_vv[:, u2, :])
+        w0 = np.einsum("xd,zyd->xyz", ovvv, inp.t2[:, :, u3, :], optimize=True)
+        # hole:   - sum_l (x1 u1|x2 l) t2[l,x3,u2,u3]
+        ovoo = np.einsum("Qx,Qyl->xyl", inp.B_ov[:, :, u1], inp.B_oo, optimize=True)
+        w0 -= np.einsum("xyl,lz->xyz", ovoo, inp.t2[:, :, u2, u3], optimize=True)
+        # w0 is indexed [x1,x2,x3]; x_m is the occupied paired with vir[perm[m]],
+        # i.e. axis m of w0 is axis perm[m] of W[i,j,k].
+        W += np.transpose(w0, np.argsort(perm))
+    return W
+
+
+def v_virtual_triple(inp, a, b, c, W):
+    """V^{abc}[i,j,k] = W + t1 (ov|ov) terms (+ the Fock term), Eqs. (5)-(7)."""
+    t1 = inp.t1
+    J = lambda u, w: np.einsum("Qx,Qy->xy", inp.B_ov[:, :, u], inp.B_ov[:, :, w])  # (x u|y w)
+    V = W.copy()
+    V += t1[:, a][:, None, None] * J(b, c)[None, :, :]
+    V += t1[:, b][None, :, None] * J(a, c)[:, None, :]
+    V += t1[:, c][None, None, :] * J(a, b)[:, :, None]
+    f = getattr(inp, "f_ov", None)
+    if f is not None:
+        V += f[:, a][:, None, None] * inp.t2[:, :, b, c][None, :, :]
+        V += f[:, b][None, :, None] * inp.t2[:, :, a, c][:, None, :]
+        V += f[:, c][None, None, :] * inp.t2[:, :, a, b][:, :, None]
+    return V
+
+
+def e_virtual_triple(inp, a, b, c, with_t1=True):
+    """(2/alpha) sum_ijk r3_ijk(W) V / D for a<=b<=c: the abc-driven contribution."""
+    assert a <= b <= c
+    W = w_virtual_triple(inp, a, b, c)
+    V = v_virtual_triple(inp, a, b, c, W) if with_t1 else W
+    e = inp.eps_occ
+    D = (e[:, None, None] + e[None, :, None] + e[None, None, :]
+         - inp.eps_vir[a] - inp.eps_vir[b] - inp.eps_vir[c])
+    alpha = 6.0 if a == b == c else (2.0 if (a == b or b == c) else 1.0)
+    x = r_of_w(W) * V / D
+    return (2.0 / alpha) * float(np.sum(x.astype(np.longdouble)))
+
+
+def t_energy_abc(inp, with_t1=True, return_triples=False):
+    """E(T) by the abc-driven loop, summed in virtual-triple index order."""
+    trip = triplet_list(inp.nvir)
+    e = np.zeros(len(trip))
+    for n, (a, b, c) in enumerate(trip):
+        e[n] = e_virtual_triple(inp, a, b, c, with_t1)
+    total = float(np.sum(e.astype(np.longdouble)))
+    return (total, e) if return_triples else total
 
 
 # --------------------------------------------------------------------------
