@@ -42,7 +42,12 @@ def parse():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=5, help="BASELINE.json configs[n-1], n = 1..5")
+    ap.add_argument("--config", type=int, default=5,
+                    help="BASELINE.json configs[n-1], n = 1..5; 6-8 = cc-pVTZ/QZ-shaped inputs (SURVEY NEXT-2)")
+    ap.add_argument("--schedule", default="ijk", choices=["ijk", "abc"],
+                    help="ijk: occupied triplets outside, v^3 inside (default); abc: the paper's loop order, "
+                         "virtual triples outside, o^3 inside (BQC_T_FLAG_ABC_DRIVEN)")
+    ap.add_argument("--abc-window", type=int, default=38, help="virtual orbitals per triple block (--schedule abc)")
     ap.add_argument("--window", type=int, default=10, help="occupied orbitals per triplet block (per GPU)")
     ap.add_argument("--full", action="store_true", help="whole E(T) of the config in one step")
     ap.add_argument("--occ-block", type=int, default=0)
@@ -55,8 +60,12 @@ def parse():
     return ap.parse_args()
 
 
-def workload_name(cfg, c, lo, hi, full, ntrip):
+def workload_name(cfg, c, lo, hi, full, ntrip, abc=False):
     base = f"config{cfg} nocc={c['nocc']} nvir={c['nvir']} naux={c['naux']} (synthetic water-cluster shape)"
+    if abc:
+        if full:
+            return base + f", abc-driven schedule, full E(T): all {ntrip} virtual triples a<=b<=c"
+        return base + f", abc-driven schedule, one triple block per GPU: virtual window [{lo},{hi}) = {ntrip} triples"
     if full:
         return base + f", full E(T): all {ntrip} triplets i<=j<=k"
     return base + f", one triplet block per GPU: occupied window [{lo},{hi}) = {ntrip} triplets"
@@ -116,11 +125,12 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------- reference arm (oracle)
-def oracle_sample(inp, triplet):
-    """Time the oracle as it stands on one triplet of the workload; returns (seconds, e_ijk)."""
+def oracle_sample(inp, triplet, abc=False):
+    """Time the oracle as it stands on one triplet (one virtual triple for the abc-driven schedule) of the
+    workload; returns (seconds, e_ijk)."""
     from oracle import t_oracle as orc      # bench.py's cpu_baseline / --impl reference leg only
     t0 = time.perf_counter()
-    e = orc.e_triplet(inp, *triplet)
+    e = orc.e_virtual_triple(inp, *triplet) if abc else orc.e_triplet(inp, *triplet)
     return time.perf_counter() - t0, e
 
 
@@ -265,17 +275,20 @@ def main():
 
     c = CONFIGS[args.config]
     o, v, X = c["nocc"], c["nvir"], c["naux"]
-    w = o if args.full else min(args.window, o)
-    nblocks = max(1, o // w)
+    abc = args.schedule == "abc"
+    nidx = v if abc else o                  # the index the outer loop (window, blocks, shards) runs over
+    sched_flags = bqc.BQC_T_FLAG_PROFILE | (bqc.BQC_T_FLAG_ABC_DRIVEN if abc else 0)
+    w = nidx if args.full else min(args.abc_window if abc else args.window, nidx)
+    nblocks = max(1, nidx // w)
     lo = 0 if args.full else (rank % nblocks) * w
-    hi = o if args.full else lo + w
+    hi = nidx if args.full else lo + w
     if args.full and world > 1:
-        opts = bqc.make_opts(occ_block=args.occ_block, shard_rank=rank, shard_count=world,
-                             flags=bqc.BQC_T_FLAG_PROFILE)
+        opts = bqc.make_opts(occ_block=args.occ_block, shard_rank=rank, shard_count=world, flags=sched_flags)
     else:
-        opts = bqc.make_opts(occ_block=args.occ_block, occ_lo=lo, occ_hi=hi, flags=bqc.BQC_T_FLAG_PROFILE)
+        opts = bqc.make_opts(occ_block=args.occ_block, occ_lo=lo, occ_hi=hi, flags=sched_flags)
     flops_rank = bqc.bqc_t_flops(o, v, opts)
-    ntrip = int(round(flops_rank / (12.0 * v ** 3 * (v + o))))
+    f1 = 12.0 * o ** 3 * (v + o) if abc else 12.0 * v ** 3 * (v + o)      # flops of one unit of the outer loop
+    ntrip = int(round(flops_rank / f1))
 
     t0 = time.perf_counter()
     inp = make_config(args.config)
@@ -298,7 +311,7 @@ def main():
     # FP64 tensor-core peak measured in this run: the roofline denominator
     peak_dmma = bqc.bqc_fp64_peak_tflops(0, args.peak_seconds)
 
-    e_trip = torch.zeros(bqc.bqc_t_num_triplets(o), dtype=torch.float64, device="cuda")
+    e_trip = torch.zeros(bqc.bqc_t_num_triplets(nidx), dtype=torch.float64, device="cuda")
 
     def step():
         return bqc.bqc_t_energy_ex(o, v, X, *dev, opts=opts, workspace=ws, e_triplet=e_trip)
@@ -329,7 +342,8 @@ def main():
         del ws
         torch.cuda.empty_cache()
         eopts = bqc.make_opts(occ_block=args.occ_block, occ_lo=opts.occ_lo, occ_hi=opts.occ_hi,
-                              shard_rank=opts.shard_rank, shard_count=opts.shard_count)
+                              shard_rank=opts.shard_rank, shard_count=opts.shard_count,
+                              flags=bqc.BQC_T_FLAG_ABC_DRIVEN if abc else 0)
         barrier()
         t0 = time.perf_counter()
         for _ in range(args.e2e_steps):
@@ -354,14 +368,14 @@ def main():
 
     if rank == 0:
         value = flops_total / (ms * 1e-3) * 1e-12
-        flops_full = bqc.bqc_t_flops(o, v)
+        flops_full = bqc.bqc_t_flops(o, v, bqc.make_opts(flags=bqc.BQC_T_FLAG_ABC_DRIVEN) if abc else None)
         gemm_tf = flops_rank / (prof["gemm_ms"] * 1e-3) * 1e-12 if prof["gemm_ms"] > 0 else None
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(args.config, c, lo, hi, args.full, ntrip),
-                       "triplets_per_gpu": ntrip, "occ_block": bqc.bqc_t_plan_occ_block(o, v, X, opts),
+            "config": {"workload": workload_name(args.config, c, lo, hi, args.full, ntrip, abc),
+                       "schedule": args.schedule, "triplets_per_gpu": ntrip, "occ_block": bqc.bqc_t_plan_occ_block(o, v, X, opts),
                        "l2": "inputs larger than L2 (554 MB augmented slabs, 1.4 GB F per triplet); no flush needed"
                              if args.config >= 4 else "working set may fit L2 on small configs",
                        "timing": "CUDA events on the launch stream around K bqc_t_energy_ex calls, max over ranks",
@@ -381,9 +395,10 @@ def main():
                                         "mma.sync m8n8k4 loop on all SMs); MEASURED_PEAKS.json has no FP64 entry",
                          "launches": int(prof["gemm_launches"]),
                          "flops_per_launch": flops_rank / max(prof["gemm_launches"], 1),
-                         "traffic": NCU_TRAFFIC_W_BUILDER.get(args.config),
+                         "traffic": None if abc else NCU_TRAFFIC_W_BUILDER.get(args.config),
                          "traffic_source": "ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch "
-                                           "(profiles/r1b_gemm_nt_full.txt)" if args.config in NCU_TRAFFIC_W_BUILDER
+                                           "(profiles/r1b_gemm_nt_full.txt)" if (args.config in NCU_TRAFFIC_W_BUILDER
+                                                                                   and not abc)
                                            else None},
             "clocks": clocks,
             "e2e": {"value": (flops_total / (e2e_ms_max * 1e-3) * 1e-12) if e2e_ms_max else None, "unit": UNIT,
@@ -396,13 +411,12 @@ def main():
             # per-triplet values are compared with the e_ijk the timed GPU steps produced (north_star tolerance)
             mid = (lo + hi - 1) // 2
             trips = [(lo, mid, hi - 1), (lo, lo, hi - 1), (lo, hi - 1, hi - 1)][:max(1, args.cpu_triplets)]
-            f1 = 12.0 * v ** 3 * (v + o)
             e_gpu = e_trip.cpu().numpy()
             dts, worst = [], 0.0
             for trip in trips:
-                dt, e_ref = oracle_sample(inp, trip)
+                dt, e_ref = oracle_sample(inp, trip, abc)
                 dts.append(dt)
-                d = abs(e_gpu[bqc.bqc_t_triplet_index(o, *trip)] - e_ref)
+                d = abs(e_gpu[bqc.bqc_t_triplet_index(nidx, *trip)] - e_ref)
                 worst = max(worst, d / (1e-10 * abs(e_ref) + 1e-12 * abs(e_total) / max(ntrip, 1)))
             dt = float(np.sum(dts))
             out["cpu_baseline"] = {"value": len(trips) * f1 / dt * 1e-12, "unit": UNIT, "cores": cpu_threads(),

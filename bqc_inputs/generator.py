@@ -57,6 +57,12 @@ CONFIGS = {
     3: dict(nocc=40, nvir=152, naux=672, t2_std=1e-2, seed=1003),
     4: dict(nocc=80, nvir=304, naux=1344, t2_std=5e-3, seed=1004),
     5: dict(nocc=100, nvir=380, naux=1680, t2_std=5e-3, seed=1005),
+    # larger-basis shapes (same generator).  The paper's water clusters in
+    # cc-pVTZ / cc-pVQZ have 58 / 115 orbitals and 5 occupied per water (8.6 % / 4.3 %
+    # occupied); naux = 3.5 x orbitals as in configs 1-5.
+    6: dict(nocc=20, nvir=212, naux=812, t2_std=1e-2, seed=1006),    # 4 waters, cc-pVTZ-shaped
+    7: dict(nocc=10, nvir=220, naux=805, t2_std=1e-2, seed=1007),    # 2 waters, cc-pVQZ-shaped
+    8: dict(nocc=40, nvir=424, naux=1624, t2_std=5e-3, seed=1008),   # 8 waters, cc-pVTZ-shaped
 }
 
 
@@ -99,7 +105,7 @@ def make_inputs(nocc: int, nvir: int, naux: int, seed: int,
 
 
 def make_config(idx: int, **overrides) -> TInputs:
-    """BASELINE.json configs[idx-1] (idx = 1..5)."""
+    """BASELINE.json configs[idx-1] (idx = 1..5); idx = 6..8: the larger-basis shapes of NEXT-2."""
     c = dict(CONFIGS[idx])
     c.update(overrides)
     return make_inputs(c["nocc"], c["nvir"], c["naux"], c["seed"],

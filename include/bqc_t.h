@@ -78,8 +78,21 @@ typedef struct bqc_t_opts {
 
 enum {
   BQC_T_FLAG_NO_T1 = 1,         /* drop the t1 (E[5]) and Fock terms: V = W (E[4]-only checks) */
-  BQC_T_FLAG_PROFILE = 2        /* bracket every kernel group with CUDA events on its launching
+  BQC_T_FLAG_PROFILE = 2,       /* bracket every kernel group with CUDA events on its launching
                                    stream; read the sums with bqc_t_last_profile             */
+  BQC_T_FLAG_ABC_DRIVEN = 4     /* abc-driven schedule (the paper's loop order; SURVEY.md
+                                   §8(f) NEXT-2): the outer loop runs over virtual triples a<=b<=c with all
+                                   o^3 occupied triples inside, instead of occupied triplets i<=j<=k with
+                                   all v^3 virtual triples inside.  Same E(T) up to summation order; the
+                                   resident pieces are o^2 (v+o) per virtual instead of v^2 (v+o) per
+                                   occupied orbital, which is what large virtual spaces (cc-pVTZ/QZ-shaped
+                                   inputs) need.  With this flag occ_block / occ_lo / occ_hi / shard_* refer
+                                   to the VIRTUAL index, e_triplet_dev has bqc_t_num_triplets(nvir) entries
+                                   indexed by bqc_t_triplet_index(nvir, a, b, c) and holds the weighted
+                                   per-virtual-triple contributions (2 - d_ab - d_bc) sum_ijk R V / D, and
+                                   bqc_t_flops counts 12 o^3 (v+o) per virtual triple.  The library builds
+                                   the transposed amplitude / DF arrays it needs inside the workspace
+                                   (one extra copy of t2 and B_ov).                                      */
 };
 
 /* ---- host-only helpers (no GPU needed) -------------------------------------------------- */

@@ -35,6 +35,7 @@ class bqc_mp2_opts(Structure):
 
 BQC_T_FLAG_NO_T1 = 1
 BQC_T_FLAG_PROFILE = 2
+BQC_T_FLAG_ABC_DRIVEN = 4
 
 _lib = None
 
@@ -153,6 +154,12 @@ def _optp(opts):
 
 
 # ---------------------------------------------------------------- host-only helpers
+def _ntrip_out(nocc, nvir, opts):
+    """Length of the per-triplet output: occupied triplets, or virtual triples under BQC_T_FLAG_ABC_DRIVEN."""
+    abc = opts is not None and (opts.flags & BQC_T_FLAG_ABC_DRIVEN)
+    return bqc_t_num_triplets(nvir if abc else nocc)
+
+
 def bqc_t_num_triplets(nocc):
     return lib().bqc_t_num_triplets(nocc)
 
@@ -207,14 +214,15 @@ def bqc_t_energy(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv):
 def bqc_t_energy_ex(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, opts=None,
                     workspace=None, e_triplet=None):
     """Returns E (this shard / window).  `workspace`: optional uint8 CUDA tensor;
-    `e_triplet`: optional float64 CUDA tensor [num_triplets] filled with e_ijk."""
+    `e_triplet`: optional float64 CUDA tensor [num_triplets] filled with e_ijk
+    (e_abc over virtual triples, [num_triplets(nvir)], under BQC_T_FLAG_ABC_DRIVEN)."""
     p = _inputs(nocc, nvir, naux, (eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv), True)
     ws_ptr, ws_bytes = None, 0
     if workspace is not None:
         ws_ptr, ws_bytes = c_void_p(workspace.data_ptr()), workspace.numel() * workspace.element_size()
     et = None
     if e_triplet is not None:
-        et = _ptr(e_triplet, (bqc_t_num_triplets(nocc),), "e_triplet", True)
+        et = _ptr(e_triplet, (_ntrip_out(nocc, nvir, opts),), "e_triplet", True)
     e = c_double(0.0)
     _check(lib().bqc_t_energy_ex(nocc, nvir, naux, *p, _optp(opts), ws_ptr, ws_bytes, byref(e), et,
                                  _stream()))
@@ -236,7 +244,7 @@ def bqc_t_energy_host(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_
     p = _inputs(nocc, nvir, naux, (eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv), False)
     et = None
     if e_triplet is not None:
-        et = _ptr(e_triplet, (bqc_t_num_triplets(nocc),), "e_triplet", False)
+        et = _ptr(e_triplet, (_ntrip_out(nocc, nvir, opts),), "e_triplet", False)
     e = c_double(0.0)
     h2d, d2h = c_size_t(0), c_size_t(0)
     _check(lib().bqc_t_energy_host(nocc, nvir, naux, *p, _optp(opts), byref(e), et, byref(h2d),

@@ -7,6 +7,10 @@ namespace bqc {
 // out[r][q] (pitch qp, zero for q >= nq) = in[q][r]        (in: [nq][nr] row-major)
 int launch_transpose_pad(const double* in, double* out, int nq, int nr, int qp, cudaStream_t s);
 
+// out[b][c][r] = scale * in[b][r][c]   (in: [batch][nr][nc] row-major; nr <= 32*65535, batch <= 65535)
+int launch_transpose_scale(const double* in, double* out, int batch, long long nr, long long nc, double scale,
+                           cudaStream_t s);
+
 // Btil[pz*na + py][r][d] = t2[act[pz]][act[py]][r][d], d < v  (row pitch kp).  Columns >= v untouched.
 int launch_btilde_t2(const double* t2, double* btil, int o, int v, const int* act_dev, int na, int kp,
                      cudaStream_t s);

@@ -28,6 +28,40 @@ int launch_transpose_pad(const double* in, double* out, int nq, int nr, int qp, 
   return BQC_OK;
 }
 
+// ---------------------------------------------------------------- out[b][c][r] = scale * in[b][r][c]
+// (the particle-hole dual arrays of the abc-driven schedule, t_energy.cu)
+__global__ void transpose_scale_kernel(const double* __restrict__ in, double* __restrict__ out, long long nr,
+                                       long long nc, double scale) {
+  __shared__ double tile[32][33];
+  const long long c0 = (long long)blockIdx.x * 32, r0 = (long long)blockIdx.y * 32;
+  const double* src = in + (size_t)blockIdx.z * nr * nc;
+  double* dst = out + (size_t)blockIdx.z * nr * nc;
+  for (int dy = threadIdx.y; dy < 32; dy += blockDim.y) {
+    const long long r = r0 + dy, c = c0 + threadIdx.x;
+    tile[dy][threadIdx.x] = (r < nr && c < nc) ? src[r * nc + c] : 0.0;
+  }
+  __syncthreads();
+  for (int dy = threadIdx.y; dy < 32; dy += blockDim.y) {
+    const long long c = c0 + dy, r = r0 + threadIdx.x;
+    if (c < nc && r < nr) dst[c * nr + r] = scale * tile[threadIdx.x][dy];
+  }
+}
+
+int launch_transpose_scale(const double* in, double* out, int batch, long long nr, long long nc, double scale,
+                           cudaStream_t s) {
+  const long long gx = (nc + 31) / 32, gy = (nr + 31) / 32;
+  if (batch <= 0 || nr <= 0 || nc <= 0) return BQC_OK;
+  if (gy > 65535 || batch > 65535 || gx > 2147483647LL) {
+    set_error(BQC_ERR_INVALID_SIZE, "transpose of %d x %lld x %lld exceeds the launch grid", batch, nr, nc);
+    return BQC_ERR_INVALID_SIZE;
+  }
+  transpose_scale_kernel<<<dim3((unsigned)gx, (unsigned)gy, (unsigned)batch), dim3(32, 8), 0, s>>>(in, out, nr, nc,
+                                                                                                   scale);
+  count_launch();
+  BQC_CUDA_OK(cudaGetLastError());
+  return BQC_OK;
+}
+
 // ---------------------------------------------------------------- t2 rows -> Btilde rows
 __global__ void btilde_t2_kernel(const double* __restrict__ t2, double* __restrict__ btil, int o, int v,
                                  const int* __restrict__ act, int na, int kp) {

@@ -768,6 +768,103 @@ int t_energy_impl(int o, int v, int X, const Inputs& in, const bqc_t_opts* opts,
   return BQC_OK;
 }
 
+// ------------------------------------------------------------------ abc-driven schedule
+// The paper's loop is over virtual triples a,b,c with o^3 tensors per iteration.  The
+// contraction of Eq. (2) is invariant under exchanging the roles of occupied and virtual orbitals
+// (DESIGN.md §12): with
+//     o' = v, v' = o, eps_occ' = -eps_vir, eps_vir' = -eps_occ, t1'[a,i] = t1[i,a],
+//     t2'[a,b,i,j] = -t2[i,j,a,b], B_oo' = B_vv, B_vv' = B_oo, B_ov'[Q,a,i] = B_ov[Q,i,a], f'[a,i] = -f[i,a]
+// the dual problem's triplet (a <= b <= c) carries W_abc[i,j,k] for all i,j,k, its "slabs" are the o^2 (v+o)
+// pieces (zr|yl), t2[z,y,r,:] of one virtual r and its per-triplet value is the abc-driven contribution
+// (2 - d_ab - d_bc) sum_ijk R V / D.  So the abc-driven schedule is the same pipeline on the dual arrays,
+// which are built here on the device (one pass over t2 and B_ov).
+struct DualLayout {
+  size_t off_eo = 0, off_ev = 0, off_t1 = 0, off_f = 0, off_bov = 0, off_t2 = 0, total = 0;
+};
+
+DualLayout dual_layout(int o, int v, int X, bool fock) {
+  DualLayout L;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t r = off; off = round_up(off + bytes, 1024); return r; };
+  L.off_eo = take((size_t)v * 8);
+  L.off_ev = take((size_t)o * 8);
+  L.off_t1 = take((size_t)o * v * 8);
+  L.off_f = take(fock ? (size_t)o * v * 8 : 0);
+  L.off_bov = take((size_t)X * o * v * 8);
+  L.off_t2 = take((size_t)o * o * v * v * 8);
+  L.total = off;
+  return L;
+}
+
+bqc_t_opts dual_opts(const bqc_t_opts* opts) {
+  bqc_t_opts d;
+  memset(&d, 0, sizeof(d));
+  if (opts) d = *opts;
+  d.flags &= ~BQC_T_FLAG_ABC_DRIVEN;
+  d.f_ov = nullptr;
+  return d;
+}
+
+int t_energy_abc(int o, int v, int X, const Inputs& in, const bqc_t_opts* opts, void* workspace,
+                 size_t workspace_bytes, double* e_total_host, double* e_triplet_dev, cudaStream_t stream) {
+  clear_error();
+  if (!e_total_host) {
+    set_error(BQC_ERR_NULL_POINTER, "e_total_host is NULL");
+    return BQC_ERR_NULL_POINTER;
+  }
+  BQC_TRY(validate_inputs(o, v, X, in));
+  if (in.f_ov) BQC_TRY(check_device_ptr(in.f_ov, "opts->f_ov"));
+  bqc_t_opts dopts = dual_opts(opts);
+  int lo, hi;
+  BQC_TRY(resolve_window(v, &dopts, &lo, &hi));
+  Plan P;
+  {
+    std::vector<int> act(hi - lo);
+    for (int x = lo; x < hi; ++x) act[x - lo] = x;
+    BQC_TRY(make_plan(P, v, o, X, act, &dopts));
+  }
+  const DualLayout L = dual_layout(o, v, X, in.f_ov != nullptr);
+  const size_t need = L.total + P.total;
+  uint8_t* ws = static_cast<uint8_t*>(workspace);
+  bool own = false;
+  if (ws) {
+    if (workspace_bytes < need || (reinterpret_cast<uintptr_t>(ws) & 255)) {
+      set_error(BQC_ERR_WORKSPACE, "workspace of %zu bytes (need %zu, 256-byte aligned)", workspace_bytes, need);
+      return BQC_ERR_WORKSPACE;
+    }
+  } else {
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, need);
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      set_error(BQC_ERR_WORKSPACE, "cudaMalloc of %zu workspace bytes failed: %s", need, cudaGetErrorString(e));
+      return BQC_ERR_WORKSPACE;
+    }
+    ws = static_cast<uint8_t*>(p);
+    own = true;
+  }
+  auto D = [&](size_t off) { return reinterpret_cast<double*>(ws + off); };
+  const long long launches0 = g_launches;
+  int rc = launch_transpose_scale(in.eps_vir, D(L.off_eo), 1, 1, v, -1.0, stream);
+  if (rc == BQC_OK) rc = launch_transpose_scale(in.eps_occ, D(L.off_ev), 1, 1, o, -1.0, stream);
+  if (rc == BQC_OK) rc = launch_transpose_scale(in.t1, D(L.off_t1), 1, o, v, 1.0, stream);
+  if (rc == BQC_OK && in.f_ov) rc = launch_transpose_scale(in.f_ov, D(L.off_f), 1, o, v, -1.0, stream);
+  if (rc == BQC_OK) rc = launch_transpose_scale(in.B_ov, D(L.off_bov), X, o, v, 1.0, stream);
+  if (rc == BQC_OK)
+    rc = launch_transpose_scale(in.t2, D(L.off_t2), 1, (long long)o * o, (long long)v * v, -1.0, stream);
+  if (rc == BQC_OK) {
+    Inputs din = {D(L.off_eo), D(L.off_ev), D(L.off_t1), D(L.off_t2), in.B_vv, D(L.off_bov), in.B_oo,
+                  in.f_ov ? D(L.off_f) : nullptr};
+    rc = t_energy_impl(v, o, X, din, &dopts, ws + L.total, P.total, e_total_host, e_triplet_dev, stream);
+    g_profile[8] = (double)(g_launches - launches0);
+  }
+  if (own) {
+    cudaStreamSynchronize(stream);
+    cudaFree(ws);
+  }
+  return rc;
+}
+
 }  // namespace
 }  // namespace bqc
 
@@ -792,6 +889,10 @@ int bqc_t_triplet_owner(int nocc, int shard_count, int i, int j, int k) {
 double bqc_t_flops(int nocc, int nvir, const bqc_t_opts* opts) {
   clear_error();
   if (nocc <= 0 || nvir <= 0) return 0.0;
+  if (opts && (opts->flags & BQC_T_FLAG_ABC_DRIVEN)) {   // virtual triples a<=b<=c, 12 o^3 (v+o) each
+    const bqc_t_opts d = dual_opts(opts);
+    return bqc_t_flops(nvir, nocc, &d);
+  }
   int lo, hi;
   if (resolve_window(nocc, opts, &lo, &hi) != BQC_OK) return -1.0;
   const int sc = (opts && opts->shard_count > 0) ? opts->shard_count : 1;
@@ -810,6 +911,10 @@ double bqc_t_flops(int nocc, int nvir, const bqc_t_opts* opts) {
 int bqc_t_plan_occ_block(int nocc, int nvir, int naux, const bqc_t_opts* opts) {
   clear_error();
   if (check_sizes(nocc, nvir, naux) != BQC_OK) return -1;
+  if (opts && (opts->flags & BQC_T_FLAG_ABC_DRIVEN)) {   // block size over the virtual index
+    const bqc_t_opts d = dual_opts(opts);
+    return bqc_t_plan_occ_block(nvir, nocc, naux, &d);
+  }
   int lo, hi;
   if (resolve_window(nocc, opts, &lo, &hi) != BQC_OK) return -1;
   Plan P;
@@ -822,6 +927,11 @@ int bqc_t_plan_occ_block(int nocc, int nvir, int naux, const bqc_t_opts* opts) {
 size_t bqc_t_workspace_bytes(int nocc, int nvir, int naux, const bqc_t_opts* opts) {
   clear_error();
   if (check_sizes(nocc, nvir, naux) != BQC_OK) return 0;
+  if (opts && (opts->flags & BQC_T_FLAG_ABC_DRIVEN)) {   // dual arrays + the dual problem's workspace
+    const bqc_t_opts d = dual_opts(opts);
+    const size_t inner = bqc_t_workspace_bytes(nvir, nocc, naux, &d);
+    return inner ? dual_layout(nocc, nvir, naux, opts->f_ov != nullptr).total + inner : 0;
+  }
   int lo, hi;
   if (resolve_window(nocc, opts, &lo, &hi) != BQC_OK) return 0;
   Plan P;
@@ -863,6 +973,9 @@ int bqc_t_energy_ex(int nocc, int nvir, int naux, const double* eps_occ, const d
                     const double* B_vv, const bqc_t_opts* opts, void* workspace, size_t workspace_bytes,
                     double* e_total_host, double* e_triplet_dev, void* stream) {
   Inputs in = {eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, opts ? opts->f_ov : nullptr};
+  if (opts && (opts->flags & BQC_T_FLAG_ABC_DRIVEN))
+    return t_energy_abc(nocc, nvir, naux, in, opts, workspace, workspace_bytes, e_total_host, e_triplet_dev,
+                        static_cast<cudaStream_t>(stream));
   return t_energy_impl(nocc, nvir, naux, in, opts, workspace, workspace_bytes, e_total_host, e_triplet_dev,
                        static_cast<cudaStream_t>(stream));
 }
@@ -900,7 +1013,8 @@ int bqc_t_energy_host(int nocc, int nvir, int naux, const double* eps_occ, const
   }
   size_t total = 0, offs[8];
   for (int n = 0; n < nin; ++n) { offs[n] = total; total += round_up(elems[n] * 8, 256); }
-  const size_t ntrip = num_triplets(nocc);
+  const bool abc = opts && (opts->flags & BQC_T_FLAG_ABC_DRIVEN);
+  const size_t ntrip = num_triplets(abc ? nvir : nocc);
   const size_t off_trip = total;
   total += round_up(ntrip * 8, 256);
   uint8_t* dev = nullptr;
