@@ -69,6 +69,23 @@ int choose_nf(long long n_ext) {
   return best;
 }
 
+int split_n(int n_ext, NSegment seg[2]) {
+  const int g = (n_ext + 15) / 16;                       // 16-column groups to cover
+  if (g <= kMaxNF) {
+    seg[0] = {0, 1, g < kMinNF ? kMinNF : g};
+    return 1;
+  }
+  const int k = (g + kMaxNF - 1) / kMaxNF;               // fewest tiles
+  const int lo = g / k, nhi = g % k;                     // nhi tiles of lo+1 groups, the rest lo  (lo >= kMinNF)
+  if (nhi == 0) {
+    seg[0] = {0, k, lo};
+    return 1;
+  }
+  seg[0] = {0, nhi, lo + 1};
+  seg[1] = {nhi * 16 * (lo + 1), k - nhi, lo};
+  return 2;
+}
+
 void choose_m_tile(int m1_ext, int m2_ext, int* tp, int* tq_log2) {
   long long best_cost = -1;
   for (int lg = 7; lg >= 3; --lg) {   // tq = 128 ... 8 (a TMA sub-box of tq rows must span whole 1 KiB swizzle atoms)
@@ -76,6 +93,31 @@ void choose_m_tile(int m1_ext, int m2_ext, int* tp, int* tq_log2) {
     const long long cost = (long long)round_up_i(m1_ext, tpp) * round_up_i(m2_ext, tq);
     if (best_cost < 0 || cost < best_cost) { best_cost = cost; *tp = tpp; *tq_log2 = lg; }
   }
+}
+
+int split_m(int m1_ext, int m2_ext, MSegment seg[2]) {
+  long long best = -1;
+  int nbest = 0;
+  for (int lg = 7; lg >= 3; --lg) {
+    const int tq = 1 << lg, tp = kBM / tq;
+    const int main_tiles = m1_ext / tp, r = m1_ext - main_tiles * tp;
+    long long cost = (long long)main_tiles * tp * round_up_i(m2_ext, tq);
+    MSegment cand[2];
+    int n = 0;
+    if (main_tiles > 0) cand[n++] = {0, main_tiles, tp, lg};
+    if (r > 0) {
+      int stp = 0, slg = 0;
+      choose_m_tile(r, m2_ext, &stp, &slg);
+      cost += (long long)round_up_i(r, stp) * round_up_i(m2_ext, 1 << slg);
+      cand[n++] = {main_tiles * tp, ceil_div(r, stp), stp, slg};
+    }
+    if (best < 0 || cost < best) {
+      best = cost;
+      nbest = n;
+      for (int k = 0; k < n; ++k) seg[k] = cand[k];
+    }
+  }
+  return nbest;
 }
 
 template <int NF>

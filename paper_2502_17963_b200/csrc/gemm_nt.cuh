@@ -52,6 +52,7 @@ struct GemmParams {
   int tiles_m1, tiles_m2, tiles_n;   // per task
   int tp, tq_log2;                   // M tile = tp (m1) x tq (m2), tq = 1 << tq_log2
   int m1_base, n_base;               // added to the TMA coordinates (not to the output index)
+  int m1_out, n_out;                 // added to the output index (a launch may cover a sub-range of M1 / N)
   int m1_ext, m2_ext, n_ext;         // valid extents of the output index ranges
   int kiters;                        // ceil(K / 16) per term
   // output addressing
@@ -220,9 +221,9 @@ gemm_nt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     }
 
     // ------------------------------- epilogue: registers -> global -------------------------------
-    const int m1_0 = m1_t * prm.tp;
+    const int m1_0 = prm.m1_out + m1_t * prm.tp;
     const int m2_0 = m2_t * tq;
-    const int n_0 = n_t * kBN + warp_n0 + 2 * t;
+    const int n_0 = prm.n_out + n_t * kBN + warp_n0 + 2 * t;
     double* __restrict__ C = prm.C + task->c_off;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -275,8 +276,18 @@ int launch_gemm_nt(int nf, const CUtensorMap& tmA, const CUtensorMap& tmAT, cons
                    const GemmParams& prm, cudaStream_t stream);
 // NF that minimises padded work for an N extent (ties -> larger tile).
 int choose_nf(long long n_ext);
+// Cover [0, n_ext) with the fewest column tiles of 16*NF, NF in [kMinNF, kMaxNF], spreading the slack evenly
+// so that the padded extent is n_ext rounded up to 16 whenever n_ext >= 16*kMinNF.  At most two distinct NF
+// values result; tiles of equal NF are adjacent.  Returns the number of segments written (<= 2).
+struct NSegment { int n0, ntiles, nf; };
+int split_n(int n_ext, NSegment seg[2]);
 // (tp, tq_log2) with tp * tq = 128 minimising padded rows for extents (m1_ext, m2_ext).
 void choose_m_tile(int m1_ext, int m2_ext, int* tp, int* tq_log2);
+
+// Cover the M index pairs [0, m1_ext) x [0, m2_ext) with a main range of full (tp x tq) tiles and, if m1_ext is
+// not a multiple of tp, a strip of the remaining m1 rows with its own tile shape, minimising padded rows.
+struct MSegment { int m1_0, tiles_m1, tp, tq_log2; };
+int split_m(int m1_ext, int m2_ext, MSegment seg[2]);
 
 int device_sm_count();
 

@@ -233,8 +233,11 @@ struct Ctx {
   bool ev_free_valid[4] = {};
   int set_block[4] = {-1, -1, -1, -1};
   // F-GEMM configuration
-  int f_tp = 1, f_tq_log2 = 7, f_nf = 8;
-  CUtensorMap tm_slab, tm_slabT, tm_btil;
+  MSegment f_mseg[2];                // row segments of the F GEMM (split_m): main tiles + remainder strip
+  int f_nmseg = 0;
+  NSegment f_seg[2];                 // column segments of the F GEMM (split_n): exact cover of v up to 16
+  int f_nseg = 0;
+  CUtensorMap tm_slab[2], tm_slabT[2], tm_btil[2];
   // host schedule
   std::vector<GemmTask> tasks;
   std::vector<TripletRec> trips;
@@ -414,12 +417,38 @@ int Pipeline::setup(int o, int v, int X, const Inputs& in, const std::vector<int
   BQC_CUDA_OK(cudaEventCreateWithFlags(&c.ev_join, cudaEventDisableTiming));
 
   const Plan& P = c.P;
-  choose_m_tile(v, v, &c.f_tp, &c.f_tq_log2);
-  c.f_nf = choose_nf(v);
-  const int tq = 1 << c.f_tq_log2;
-  BQC_TRY(tmap(&c.tm_slab, c.slabs(), P.Kp, v, v, P.nslots, tq, c.f_tp));
-  BQC_TRY(tmap(&c.tm_slabT, c.slabs(), P.Kp, v, v, P.nslots, 1, tq));
-  BQC_TRY(tmap(&c.tm_btil, c.btil(), P.Kp, v, (unsigned long long)P.na * P.na, 1, gemm_bn(c.f_nf), 1));
+  c.f_nmseg = split_m(v, v, c.f_mseg);
+  c.f_nseg = split_n(v, c.f_seg);
+  for (int m = 0; m < c.f_nmseg; ++m) {
+    const int tq = 1 << c.f_mseg[m].tq_log2;
+    BQC_TRY(tmap(&c.tm_slab[m], c.slabs(), P.Kp, v, v, P.nslots, tq, c.f_mseg[m].tp));
+    BQC_TRY(tmap(&c.tm_slabT[m], c.slabs(), P.Kp, v, v, P.nslots, 1, tq));
+  }
+  for (int n = 0; n < c.f_nseg; ++n)
+    BQC_TRY(tmap(&c.tm_btil[n], c.btil(), P.Kp, v, (unsigned long long)P.na * P.na, 1, gemm_bn(c.f_seg[n].nf), 1));
+  return BQC_OK;
+}
+
+// The W-builder GEMM of `prm.ntasks` tasks: one launch per (row segment, column segment).
+int launch_f_gemm(Ctx& c, GemmParams prm, cudaStream_t s) {
+  const int v = c.P.v;
+  prm.m1_ext = v; prm.m2_ext = v; prm.n_ext = v;
+  prm.kiters = c.P.Kp / kBK;
+  prm.out_mode = 1;
+  prm.nbv = c.P.nbv;
+  prm.n2_ext = 1;
+  for (int m = 0; m < c.f_nmseg; ++m) {
+    const MSegment& ms = c.f_mseg[m];
+    prm.tp = ms.tp; prm.tq_log2 = ms.tq_log2;
+    prm.tiles_m1 = ms.tiles_m1;
+    prm.tiles_m2 = ceil_div(v, 1 << ms.tq_log2);
+    prm.m1_base = prm.m1_out = ms.m1_0;
+    for (int n = 0; n < c.f_nseg; ++n) {
+      prm.tiles_n = c.f_seg[n].ntiles;
+      prm.n_base = prm.n_out = c.f_seg[n].n0;
+      BQC_TRY(launch_gemm_nt(c.f_seg[n].nf, c.tm_slab[m], c.tm_slabT[m], c.tm_btil[n], prm, s));
+    }
+  }
   return BQC_OK;
 }
 
@@ -615,19 +644,10 @@ int Pipeline::compute(const Action& a) {
   GemmParams prm;
   memset(&prm, 0, sizeof(prm));
   prm.ntasks = (int)(3 * a.ntrip);
-  prm.tp = c.f_tp; prm.tq_log2 = c.f_tq_log2;
-  prm.tiles_m1 = ceil_div(v, c.f_tp);
-  prm.tiles_m2 = ceil_div(v, 1 << c.f_tq_log2);
-  prm.tiles_n = ceil_div(v, gemm_bn(c.f_nf));
-  prm.m1_ext = v; prm.m2_ext = v; prm.n_ext = v;
-  prm.kiters = P.Kp / kBK;
-  prm.out_mode = 1;
-  prm.nbv = P.nbv;
-  prm.n2_ext = 1;
   prm.tasks = c.tasks_dev() + a.task0;
   prm.C = c.F();
   if (P.profile) BQC_TRY(c.prof_mark(c.prof_main, s));
-  BQC_TRY(launch_gemm_nt(c.f_nf, c.tm_slab, c.tm_slabT, c.tm_btil, prm, s));
+  BQC_TRY(launch_f_gemm(c, prm, s));
   if (P.profile) BQC_TRY(c.prof_mark(c.prof_main, s));
 
   EnergyArgs e;
@@ -1169,18 +1189,9 @@ int bqc_t_debug_wv(int nocc, int nvir, int naux, const double* eps_occ, const do
   GemmParams prm;
   memset(&prm, 0, sizeof(prm));
   prm.ntasks = 3;
-  prm.tp = c.f_tp; prm.tq_log2 = c.f_tq_log2;
-  prm.tiles_m1 = ceil_div(nvir, c.f_tp);
-  prm.tiles_m2 = ceil_div(nvir, 1 << c.f_tq_log2);
-  prm.tiles_n = ceil_div(nvir, gemm_bn(c.f_nf));
-  prm.m1_ext = nvir; prm.m2_ext = nvir; prm.n_ext = nvir;
-  prm.kiters = P.Kp / kBK;
-  prm.out_mode = 1;
-  prm.nbv = P.nbv;
-  prm.n2_ext = 1;
   prm.tasks = c.tasks_dev() + task0;
   prm.C = c.F();
-  BQC_TRY(launch_gemm_nt(c.f_nf, c.tm_slab, c.tm_slabT, c.tm_btil, prm, stream));
+  BQC_TRY(launch_f_gemm(c, prm, stream));
   BQC_TRY(launch_assemble_wv(c.F(), P.nbv, nvir, c.J(), P.na, pi, pj, pk, t1 + (size_t)i * nvir,
                              t1 + (size_t)j * nvir, t1 + (size_t)k * nvir, t2, nocc, i, j, k, f_ov, W_dev, V_dev,
                              stream));

@@ -54,10 +54,11 @@ def test_df_slabs(case):
 
 
 # ------------------------------------------------------------------ rows a2 + a3: W and V
-@pytest.mark.parametrize("case", ["worked346", "config1", "ragged", "config2"])
+@pytest.mark.parametrize("case", ["worked346", "config1", "ragged", "twoseg", "config2"])
 def test_w_and_v_elementwise(case):
     inp = {"worked346": lambda: worked_example(3, 4, 6), "config1": lambda: make_config(1),
            "ragged": lambda: make_inputs(4, 35, 41, seed=8, t1_std=0.05),
+           "twoseg": lambda: make_inputs(3, 137, 21, seed=9, t1_std=0.05),   # N split into 5 + 4 groups of 16
            "config2": lambda: make_config(2, t1_std=0.05)}[case]()
     d = to_device(inp)
     o = inp.nocc
@@ -81,6 +82,8 @@ SMALL = {
     "v17": lambda: make_inputs(4, 17, 9, seed=32, t1_std=0.05),   # ragged tail of 1
     "v33": lambda: make_inputs(3, 33, 20, seed=33, t1_std=0.05),  # 3 blocks, ragged
     "o2": lambda: make_inputs(2, 9, 5, seed=34, t1_std=0.05),
+    "v137": lambda: make_inputs(3, 137, 24, seed=35, t1_std=0.05),  # 9 column groups: two GEMM column segments
+    "v209": lambda: make_inputs(2, 209, 16, seed=36, t1_std=0.05),  # 14 groups = 7 + 7, ragged 8-block tail
 }
 
 
