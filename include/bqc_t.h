@@ -158,7 +158,9 @@ BQC_API int bqc_t_last_profile(double* out, int n);
 /* End-to-end form: every array argument is a HOST pointer (pinned or pageable).  Inputs are
    copied to the device, E(T) is evaluated by the same kernels, the scalar (and, if
    e_triplet_host != NULL, the [num_triplets] per-triplet array) is copied back.
-   h2d_bytes / d2h_bytes (may be NULL) receive the bytes moved each way. */
+   With an occupied window (opts->occ_lo/occ_hi, ijk-driven schedule) only the rows t2[x,:,:,:],
+   occ_lo <= x < occ_hi, are copied: a window reads no other part of t2.
+   h2d_bytes / d2h_bytes (may be NULL) receive the bytes actually moved each way. */
 BQC_API int bqc_t_energy_host(int nocc, int nvir, int naux,
                       const double* eps_occ, const double* eps_vir,
                       const double* t1, const double* t2,

@@ -1048,13 +1048,28 @@ int bqc_t_energy_host(int nocc, int nvir, int naux, const double* eps_occ, const
   }
   int rc = BQC_OK;
   size_t h2d = 0;
+  // An occupied window [lo,hi) of the ijk-driven schedule reads t2 only through rows t2[x,:,:,:], lo <= x < hi
+  // (B~ rows, hole columns, Fock tiles): copy just that contiguous slice; the rest of the device buffer is
+  // never read.  The abc-driven schedule transposes all of t2 and takes the whole array.
+  size_t t2_first = 0, t2_count = elems[3];
+  if (!abc) {
+    int lo = 0, hi = nocc;
+    if (resolve_window(nocc, opts, &lo, &hi) != BQC_OK) {
+      cudaFree(dev);
+      return g_err;
+    }
+    t2_first = (size_t)lo * o * v * v;
+    t2_count = (size_t)(hi - lo) * o * v * v;
+  }
   for (int n = 0; n < nin && rc == BQC_OK; ++n) {
-    cudaError_t e = cudaMemcpyAsync(dev + offs[n], ptrs[n], elems[n] * 8, cudaMemcpyHostToDevice, stream);
+    const size_t first = n == 3 ? t2_first : 0, count = n == 3 ? t2_count : elems[n];
+    cudaError_t e = cudaMemcpyAsync(dev + offs[n] + first * 8, static_cast<const double*>(ptrs[n]) + first,
+                                    count * 8, cudaMemcpyHostToDevice, stream);
     if (e != cudaSuccess) {
       set_error(BQC_ERR_CUDA, "H2D copy of %s failed: %s", names[n], cudaGetErrorString(e));
       rc = BQC_ERR_CUDA;
     }
-    h2d += elems[n] * 8;
+    h2d += count * 8;
   }
   if (rc == BQC_OK) {
     auto D = [&](int n) { return reinterpret_cast<const double*>(dev + offs[n]); };
