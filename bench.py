@@ -360,9 +360,7 @@ def main():
         tsum = t.clone()
         dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
         ms, e2e_ms_max, flops_total = float(tmax[0]), float(tmax[1]), float(tsum[2])
-        esum = torch.tensor([e_val], dtype=torch.float64, device="cuda")
-        dist.all_reduce(esum, op=dist.ReduceOp.SUM)        # the path's one exchange: a scalar
-        e_total = float(esum[0])
+        e_total = bqc.combine_partials(e_val)              # the path's one exchange: a scalar per rank
     else:
         e2e_ms_max, flops_total, e_total = (e2e_ms or 0.0), float(flops_rank), e_val
 

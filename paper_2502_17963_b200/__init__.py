@@ -12,6 +12,8 @@ from .binding import (BQC_T_FLAG_NO_T1, BQC_T_FLAG_PROFILE, BQC_T_FLAG_ABC_DRIVE
                       bqc_mp2_energy, bqc_mp2_energy_ex, bqc_mp2_energy_host, bqc_mp2_flops, bqc_mp2_last_profile,
                       bqc_mp2_opts, bqc_mp2_plan_occ_block, make_mp2_opts)
 
+from .distributed import bqc_t_energy_sharded, combine_partials
+
 __all__ = [n for n in dir() if n.startswith("bqc_") or n in ("BqcError", "LIB_PATH", "lib", "make_opts", "make_mp2_opts",
                                                                "BQC_T_FLAG_NO_T1", "BQC_T_FLAG_PROFILE",
-                                                               "BQC_T_FLAG_ABC_DRIVEN")]
+                                                               "BQC_T_FLAG_ABC_DRIVEN", "combine_partials")]

@@ -233,6 +233,24 @@ def test_deterministic_and_workspace_and_host_paths():
         assert bqc.bqc_t_energy(*dims(inp), *d) == e1           # non-default stream
 
 
+def test_host_entry_point_with_a_window_copies_only_the_t2_rows_it_reads():
+    inp = make_inputs(7, 18, 13, seed=52, t1_std=0.05)
+    o, v, X = dims(inp)
+    d = to_device(inp)
+    host = [torch.from_numpy(np.ascontiguousarray(a)) for a in inp.arrays()]
+    for lo, hi in [(0, 3), (2, 6), (4, 7)]:
+        opts = bqc.make_opts(occ_lo=lo, occ_hi=hi)
+        et_d = torch.zeros(bqc.bqc_t_num_triplets(o), dtype=torch.float64, device="cuda")
+        e_dev = bqc.bqc_t_energy_ex(o, v, X, *d, opts=opts, e_triplet=et_d)
+        et_h = torch.zeros(bqc.bqc_t_num_triplets(o), dtype=torch.float64)
+        e_host, h2d, d2h = bqc.bqc_t_energy_host(o, v, X, *host, opts=opts, e_triplet=et_h)
+        assert e_host == e_dev and np.array_equal(et_h.numpy(), et_d.cpu().numpy())     # same bits
+        assert h2d == inp.nbytes() - inp.t2.nbytes + (hi - lo) * o * v * v * 8
+        # and it is the oracle's value for those triplets
+        ref = sum(orc.e_triplet(inp, i, j, k) for i in range(lo, hi) for j in range(i, hi) for k in range(j, hi))
+        assert abs(e_host - ref) <= e_tol(ref)
+
+
 # ------------------------------------------------------------------ error behaviour (no CPU fallback)
 def test_errors_are_reported():
     inp = make_config(1)

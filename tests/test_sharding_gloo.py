@@ -29,6 +29,10 @@ def _worker(rank, world, port, ret):
         if bqc.bqc_t_triplet_owner(o, world, i, j, k) == rank:
             e[bqc.bqc_t_triplet_index(o, i, j, k)] = orc.e_triplet(inp, i, j, k)
             mine += 1
+    # the library's own exchange step (paper_2502_17963_b200/distributed.py): all-gather + rank-order sum
+    from paper_2502_17963_b200.distributed import combine_partials
+    combined = combine_partials(float(e.sum()))
+    ret[f"combined{rank}"] = combined
     dist.all_reduce(e, op=dist.ReduceOp.SUM)      # disjoint supports: the sum is exact
     total = float(e.sum())
     if rank == 0:
@@ -47,4 +51,6 @@ def test_two_rank_sharded_energy_matches_single():
     ret = mgr.dict()
     mp.spawn(_worker, args=(2, port, ret), nprocs=2, join=True)
     assert ret["total"] == pytest.approx(ret["ref"], rel=1e-13)
+    assert ret["combined0"] == ret["combined1"]                      # same bits on every rank
+    assert ret["combined0"] == pytest.approx(ret["ref"], rel=1e-13)
     assert ret["count0"] + ret["count1"] == 20 and abs(ret["count0"] - ret["count1"]) <= 1
