@@ -54,6 +54,8 @@ def lib():
     L.bqc_t_num_triplets.argtypes = [c_int]
     L.bqc_t_triplet_index.restype = c_size_t
     L.bqc_t_triplet_index.argtypes = [c_int] * 4
+    L.bqc_debug_tiling.restype = c_int
+    L.bqc_debug_tiling.argtypes = [c_int, POINTER(c_int), c_int]
     L.bqc_t_triplet_owner.restype = c_int
     L.bqc_t_triplet_owner.argtypes = [c_int] * 5
     L.bqc_t_flops.restype = c_double
@@ -329,6 +331,18 @@ def bqc_t_debug_wv(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv,
     q = [c_void_p(t.data_ptr()) if t is not None else None for t in (W, V)]
     _check(lib().bqc_t_debug_wv(nocc, nvir, naux, *p, i, j, k, *q, _stream()))
     return W, V
+
+
+def bqc_debug_tiling(nvir):
+    """(column segments [(n0, ntiles, nf)], row segments [(m1_0, tiles_m1, tp, tq)]) of the W-builder GEMM."""
+    buf = (c_int * 14)()
+    rc = lib().bqc_debug_tiling(nvir, buf, 14)
+    if rc < 0:
+        _check(lib().bqc_last_error())
+    nn, nm = rc // 10, rc % 10
+    cols = [tuple(buf[3 * k:3 * k + 3]) for k in range(nn)]
+    rows = [tuple(buf[6 + 4 * k:10 + 4 * k]) for k in range(nm)]
+    return cols, rows
 
 
 def bqc_dgemm_nt(A, B, C=None):

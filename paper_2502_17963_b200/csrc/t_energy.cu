@@ -1215,6 +1215,24 @@ int bqc_t_debug_wv(int nocc, int nvir, int naux, const double* eps_occ, const do
   return BQC_OK;
 }
 
+int bqc_debug_tiling(int nvir, int* out, int n) {
+  clear_error();
+  if (nvir <= 0 || !out || n < 14) {
+    set_error(BQC_ERR_INVALID_SIZE, "bqc_debug_tiling: nvir=%d, out=%p, n=%d (need 14)", nvir, (void*)out, n);
+    return -1;
+  }
+  NSegment ns[2];
+  MSegment ms[2];
+  const int nn = split_n(nvir, ns), nm = split_m(nvir, nvir, ms);
+  for (int k = 0; k < 14; ++k) out[k] = 0;
+  for (int k = 0; k < nn; ++k) { out[3 * k] = ns[k].n0; out[3 * k + 1] = ns[k].ntiles; out[3 * k + 2] = ns[k].nf; }
+  for (int k = 0; k < nm; ++k) {
+    out[6 + 4 * k] = ms[k].m1_0; out[7 + 4 * k] = ms[k].tiles_m1; out[8 + 4 * k] = ms[k].tp;
+    out[9 + 4 * k] = 1 << ms[k].tq_log2;
+  }
+  return nn * 10 + nm;
+}
+
 int bqc_dgemm_nt(int M, int N, int K, const double* A, int lda, const double* B, int ldb, double* C, int ldc,
                  void* stream_v) {
   clear_error();

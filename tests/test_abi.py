@@ -103,3 +103,30 @@ def test_plan_and_workspace(libpath):
     assert bqc.bqc_last_error() == 9
     assert "option" in bqc.bqc_error_string(9)
     assert bqc.bqc_error_string(0) == "ok"
+
+
+def test_w_builder_tiling_covers_every_extent_exactly_once(libpath):
+    """split_n / split_m: segments are disjoint, ordered, cover [0, v) and pad as little as
+    the tile shapes allow: N to the next multiple of 16 (>= 64), M rows to v (main) + a strip < one tile."""
+    import paper_2502_17963_b200 as bqc
+    for v in list(range(1, 420)) + [512, 777, 1320]:
+        cols, rows = bqc.bqc_debug_tiling(v)
+        assert 1 <= len(cols) <= 2 and 1 <= len(rows) <= 2
+        # columns: contiguous segments, NF in [4, 8]
+        n = 0
+        for (n0, ntiles, nf) in cols:
+            assert n0 == n and ntiles >= 1 and 4 <= nf <= 8
+            n += ntiles * 16 * nf
+        assert n >= v and n == max(64, (v + 15) // 16 * 16)
+        assert sum(c[1] for c in cols) == max(1, -(-((v + 15) // 16) // 8))      # fewest tiles
+        # rows: contiguous m1 ranges, tp * tq = 128, tq >= 8
+        m = 0
+        for (m1_0, tiles_m1, tp, tq) in rows:
+            assert m1_0 == m and tiles_m1 >= 1 and tp * tq == 128 and tq >= 8
+            m += tiles_m1 * tp
+        assert m >= v
+        if len(rows) == 2:
+            assert rows[0][1] * rows[0][2] == rows[1][0] < v          # main part is all full tiles
+        padded = sum(t * tp * (-(-v // tq) * tq) for (_, t, tp, tq) in rows)
+        single = min(-(-v // (128 // tq)) * (128 // tq) * (-(-v // tq) * tq) for tq in (8, 16, 32, 64, 128))
+        assert padded <= single                                        # never worse than one tile shape
