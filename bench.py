@@ -90,6 +90,11 @@ class ClockSampler:
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
+            # nvidia-smi's own start-up briefly holds driver locks: let it reach its first sample before the
+            # timed region begins, so that short steps are not perturbed by it
+            t0 = time.perf_counter()
+            while not self.lines and time.perf_counter() - t0 < 3.0:
+                time.sleep(0.05)
         except OSError:
             self.proc = None
 

@@ -239,7 +239,7 @@ BQC_API int bqc_mp2_last_profile(double* out, int n);
 /* ---- building blocks exposed for measurement ------------------------------------------------ */
 
 /* Host-only: the tiling the W-builder GEMM uses for nvir virtual orbitals (DESIGN.md §2.3 "exact tiling").
-   out[0..5]  = up to two column segments  (n0, ntiles, NF): columns [n0, n0 + ntiles*16*NF)
+   out[0..5]  = up to two column segments  (n0, ntiles, NF): columns [n0, n0 + ntiles*8*NF)
    out[6..13] = up to two row segments     (m1_0, tiles_m1, tp, tq): rows m1 in [m1_0, m1_0 + tiles_m1*tp),
                 each tile tp (m1) x tq (m2), tp*tq = 128
    Returns 10*(number of column segments) + (number of row segments), or -1 on bad arguments (n >= 14). */

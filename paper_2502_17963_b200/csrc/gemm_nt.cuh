@@ -19,16 +19,18 @@ namespace bqc {
 
 constexpr int kBM = 128;            // rows of the A tile (= tp * tq)
 constexpr int kBK = 16;             // doubles per smem row = 128 bytes = one swizzle span
-constexpr int kConsumerWarps = 8;   // 4 (M) x 2 (N) warps, warp tile 32 x (8*NF)
+constexpr int kConsumerWarps = 8;   // 4 (M) x 2 (N) warps, warp tile 32 x (8*NF0 | 8*NF1)
 constexpr int kGemmThreads = (kConsumerWarps + 4) * 32;   // 2 consumer warpgroups + 1 producer warpgroup
-// The B tile has BN = 16*NF rows (NF = 8-column MMA fragments per warp), NF in [kMinNF, kMaxNF].
-constexpr int kMinNF = 4, kMaxNF = 8;
+// The B tile has BN = 8*NF rows: NF 8-column MMA fragments, NF0 = ceil(NF/2) owned by warp column 0 and
+// NF1 = floor(NF/2) by warp column 1 (odd NF: the last fragment of column 1 is switched off), NF in
+// [kMinNF, kMaxNF].  So any N extent is covered to within 8 columns.
+constexpr int kMinNF = 4, kMaxNF = 16;
 #ifdef __CUDACC__
 #define BQC_HD __host__ __device__
 #else
 #define BQC_HD
 #endif
-BQC_HD constexpr int gemm_bn(int nf) { return 16 * nf; }
+BQC_HD constexpr int gemm_bn(int nf) { return 8 * nf; }
 BQC_HD constexpr int gemm_stage_bytes(int nf) { return (kBM + gemm_bn(nf)) * kBK * 8; }
 BQC_HD constexpr int gemm_stages(int nf) { return (192 * 1024) / gemm_stage_bytes(nf) > 8 ? 8 : (192 * 1024) / gemm_stage_bytes(nf); }
 BQC_HD constexpr int gemm_smem_bytes(int nf) { return gemm_stages(nf) * gemm_stage_bytes(nf) + 1024 /*align slack*/ + 256 /*barriers*/; }
@@ -66,11 +68,140 @@ struct GemmParams {
 
 #ifdef __CUDACC__
 
+// b[J..N-1] = B fragment values of one k4 step (rows g + 8j of this warp's column half).
+template <int J, int N>
+__device__ __forceinline__ void load_b_frags(double (&b)[N], uint32_t pb) {
+  if constexpr (J < N) {
+    b[J] = lds_f64<J * 1024>(pb);
+    load_b_frags<J + 1, N>(b, pb);
+  }
+}
+
+// The consumer loop of one warp that owns NFW 8-column fragments starting at tile column warp_n0.
+template <int NF, int NFW>
+__device__ __forceinline__ void gemm_consume(const GemmParams& prm, uint8_t* smem, uint64_t* full_bar,
+                                             uint64_t* empty_bar, int warp, int lane, int warp_n0,
+                                             long long total_tiles, int tiles_per_task, int tq) {
+  constexpr int kBN = gemm_bn(NF);
+  constexpr int kStageBytes = gemm_stage_bytes(NF);
+  constexpr int kStages = gemm_stages(NF);
+  const int g = lane >> 2;            // fragment row (A) / column (B)
+  const int t = lane & 3;             // fragment k index
+  const int warp_m0 = (warp & 3) * 32;
+  // k slot of lane t in k4-step c is k = 2c + (t&1) + 8*(t>>1): with the 128B swizzle (16-byte chunk
+  // index ^= row & 7) the 16 lanes of a half-warp then hit 16 distinct 8-byte bank pairs.
+  uint32_t koff[4];
+#pragma unroll
+  for (int c = 0; c < 4; ++c) koff[c] = (uint32_t)((((c + 4 * (t >> 1)) ^ g) << 4) + ((t & 1) << 3));
+  const uint32_t smem_base = smem_u32(smem);
+  const uint32_t a_base = smem_base + (uint32_t)((warp_m0 + g) * (kBK * 8));
+  const uint32_t b_base = smem_base + (uint32_t)(kBM * kBK * 8 + (warp_n0 + g) * (kBK * 8));
+
+  // fragments of one k4 step: 4 A values (rows g + 8i) and NF B values (rows g + 8j), plain ld.shared
+  auto load_frags = [&](double (&a)[4], double (&b)[NFW], int stg, int c) {
+    const uint32_t off = (uint32_t)(stg * kStageBytes) + koff[c];
+    const uint32_t pa = a_base + off, pb = b_base + off;
+    a[0] = lds_f64<0 * 1024>(pa); a[1] = lds_f64<1 * 1024>(pa);
+    a[2] = lds_f64<2 * 1024>(pa); a[3] = lds_f64<3 * 1024>(pa);
+    load_b_frags<0, NFW>(b, pb);
+  };
+
+  int stage = 0;
+  uint32_t phase = 0;
+  for (long long tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+    int r = (int)(tile % tiles_per_task);
+    const int task_id = (int)(tile / tiles_per_task);
+    const int n_t = r % prm.tiles_n;  r /= prm.tiles_n;
+    const int m2_t = r % prm.tiles_m2;
+    const int m1_t = r / prm.tiles_m2;
+    const GemmTask* task = prm.tasks + task_id;
+    const int iters = task->nterms * prm.kiters;
+
+    double acc[4][NFW][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int j = 0; j < NFW; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    // Fragments are double-buffered in registers across k4 steps AND across pipeline stages: the loads
+    // of step s+1 (possibly the first step of the next stage, after its full barrier) are issued before
+    // the 4*NF DMMAs of step s, so ld.shared latency and the barrier poll hide behind tensor work.
+    double fa[2][4], fb[2][NFW];
+    mbar_wait(&full_bar[stage], phase);
+    load_frags(fa[0], fb[0], stage, 0);
+    for (int it = 0; it < iters; ++it) {
+      int nstage = stage + 1;
+      uint32_t nphase = phase;
+      if (nstage == kStages) { nstage = 0; nphase ^= 1u; }
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const int cur = c & 1, nxt = cur ^ 1;
+        if (c < 3) {
+          load_frags(fa[nxt], fb[nxt], stage, c + 1);
+        } else if (it + 1 < iters) {
+          mbar_wait(&full_bar[nstage], nphase);
+          load_frags(fa[nxt], fb[nxt], nstage, 0);
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < NFW; ++j) dmma_884(acc[i][j][0], acc[i][j][1], fa[cur][i], fb[cur][j]);
+      }
+      // every ld.shared of this stage was issued (and its value consumed by a DMMA above) -> release it
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty_bar[stage]);
+      stage = nstage;
+      phase = nphase;
+    }
+
+    // ------------------------------- epilogue: registers -> global -------------------------------
+    const int m1_0 = prm.m1_out + m1_t * prm.tp;
+    const int m2_0 = m2_t * tq;
+    const int n_0 = prm.n_out + n_t * kBN + warp_n0 + 2 * t;
+    double* __restrict__ C = prm.C + task->c_off;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int m = warp_m0 + i * 8 + g;
+      const int m1 = m1_0 + (m >> prm.tq_log2);
+      const int m2 = m2_0 + (m & (tq - 1));
+      if (m1 >= prm.m1_ext || m2 >= prm.m2_ext) continue;
+#pragma unroll
+      for (int j = 0; j < NFW; ++j) {
+        const int n = n_0 + j * 8;
+        if (n >= prm.n_ext) continue;
+        const bool has1 = (n + 1) < prm.n_ext;
+        if (prm.out_mode == 1) {
+          const long long off =
+              ((((long long)(m1 >> 3) * prm.nbv + (m2 >> 3)) * prm.nbv + (n >> 3)) << 9) +
+              ((((m1 & 7) << 3) + (m2 & 7)) << 3) + (n & 7);
+          if (has1) {
+            *reinterpret_cast<double2*>(C + off) = make_double2(acc[i][j][0], acc[i][j][1]);
+          } else {
+            C[off] = acc[i][j][0];
+          }
+        } else {
+          const long long base = (long long)m1 * prm.sM1 + (long long)m2 * prm.sM2;
+          const long long off0 = base + (long long)(n / prm.n2_ext) * prm.sN1 + (long long)(n % prm.n2_ext) * prm.sN2;
+          const long long off1 = base + (long long)((n + 1) / prm.n2_ext) * prm.sN1 +
+                                 (long long)((n + 1) % prm.n2_ext) * prm.sN2;
+          if (has1 && off1 == off0 + 1 && ((reinterpret_cast<uintptr_t>(C + off0) & 15) == 0)) {
+            *reinterpret_cast<double2*>(C + off0) = make_double2(acc[i][j][0], acc[i][j][1]);
+          } else {
+            C[off0] = acc[i][j][0];
+            if (has1) C[off1] = acc[i][j][1];
+          }
+        }
+      }
+    }
+  }
+}
+
 template <int NF>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_nt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmAT,
                const __grid_constant__ CUtensorMap tmB, const GemmParams prm) {
   constexpr int kBN = gemm_bn(NF);
+  constexpr int NF0 = (NF + 1) / 2, NF1 = NF / 2;   // fragments of warp column 0 / 1
   constexpr int kStageBytes = gemm_stage_bytes(NF);
   constexpr int kStages = gemm_stages(NF);
   extern __shared__ uint8_t smem_raw[];
@@ -145,120 +276,17 @@ gemm_nt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 
   // =============================== DMMA consumers (8 warps) ===============================
   asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
-  const int g = lane >> 2;            // fragment row (A) / column (B)
-  const int t = lane & 3;             // fragment k index
-  const int warp_m0 = (warp >> 1) * 32;
-  const int warp_n0 = (warp & 1) * (8 * NF);
-  // k slot of lane t in k4-step c is k = 2c + (t&1) + 8*(t>>1): with the 128B swizzle (16-byte chunk
-  // index ^= row & 7) the 16 lanes of a half-warp then hit 16 distinct 8-byte bank pairs.
-  uint32_t koff[4];
-#pragma unroll
-  for (int c = 0; c < 4; ++c) koff[c] = (uint32_t)((((c + 4 * (t >> 1)) ^ g) << 4) + ((t & 1) << 3));
-  const uint32_t smem_base = smem_u32(smem);
-  const uint32_t a_base = smem_base + (uint32_t)((warp_m0 + g) * (kBK * 8));
-  const uint32_t b_base = smem_base + (uint32_t)(kBM * kBK * 8 + (warp_n0 + g) * (kBK * 8));
-
-  // fragments of one k4 step: 4 A values (rows g + 8i) and NF B values (rows g + 8j), plain ld.shared
-  auto load_frags = [&](double (&a)[4], double (&b)[NF], int stg, int c) {
-    const uint32_t off = (uint32_t)(stg * kStageBytes) + koff[c];
-    const uint32_t pa = a_base + off, pb = b_base + off;
-    a[0] = lds_f64<0 * 1024>(pa); a[1] = lds_f64<1 * 1024>(pa);
-    a[2] = lds_f64<2 * 1024>(pa); a[3] = lds_f64<3 * 1024>(pa);
-    b[0] = lds_f64<0 * 1024>(pb); b[1] = lds_f64<1 * 1024>(pb);
-    b[2] = lds_f64<2 * 1024>(pb); b[3] = lds_f64<3 * 1024>(pb);
-    if (NF > 4) b[4] = lds_f64<4 * 1024>(pb);
-    if (NF > 5) b[5 % NF] = lds_f64<5 * 1024>(pb);
-    if (NF > 6) b[6 % NF] = lds_f64<6 * 1024>(pb);
-    if (NF > 7) b[7 % NF] = lds_f64<7 * 1024>(pb);
-  };
-
-  int stage = 0;
-  uint32_t phase = 0;
-  for (long long tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-    int r = (int)(tile % tiles_per_task);
-    const int task_id = (int)(tile / tiles_per_task);
-    const int n_t = r % prm.tiles_n;  r /= prm.tiles_n;
-    const int m2_t = r % prm.tiles_m2;
-    const int m1_t = r / prm.tiles_m2;
-    const GemmTask* task = prm.tasks + task_id;
-    const int iters = task->nterms * prm.kiters;
-
-    double acc[4][NF][2];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-      for (int j = 0; j < NF; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-
-    // Fragments are double-buffered in registers across k4 steps AND across pipeline stages: the loads
-    // of step s+1 (possibly the first step of the next stage, after its full barrier) are issued before
-    // the 4*NF DMMAs of step s, so ld.shared latency and the barrier poll hide behind tensor work.
-    double fa[2][4], fb[2][NF];
-    mbar_wait(&full_bar[stage], phase);
-    load_frags(fa[0], fb[0], stage, 0);
-    for (int it = 0; it < iters; ++it) {
-      int nstage = stage + 1;
-      uint32_t nphase = phase;
-      if (nstage == kStages) { nstage = 0; nphase ^= 1u; }
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const int cur = c & 1, nxt = cur ^ 1;
-        if (c < 3) {
-          load_frags(fa[nxt], fb[nxt], stage, c + 1);
-        } else if (it + 1 < iters) {
-          mbar_wait(&full_bar[nstage], nphase);
-          load_frags(fa[nxt], fb[nxt], nstage, 0);
-        }
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-#pragma unroll
-          for (int j = 0; j < NF; ++j) dmma_884(acc[i][j][0], acc[i][j][1], fa[cur][i], fb[cur][j]);
-      }
-      // every ld.shared of this stage was issued (and its value consumed by a DMMA above) -> release it
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&empty_bar[stage]);
-      stage = nstage;
-      phase = nphase;
-    }
-
-    // ------------------------------- epilogue: registers -> global -------------------------------
-    const int m1_0 = prm.m1_out + m1_t * prm.tp;
-    const int m2_0 = m2_t * tq;
-    const int n_0 = prm.n_out + n_t * kBN + warp_n0 + 2 * t;
-    double* __restrict__ C = prm.C + task->c_off;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      const int m = warp_m0 + i * 8 + g;
-      const int m1 = m1_0 + (m >> prm.tq_log2);
-      const int m2 = m2_0 + (m & (tq - 1));
-      if (m1 >= prm.m1_ext || m2 >= prm.m2_ext) continue;
-#pragma unroll
-      for (int j = 0; j < NF; ++j) {
-        const int n = n_0 + j * 8;
-        if (n >= prm.n_ext) continue;
-        const bool has1 = (n + 1) < prm.n_ext;
-        if (prm.out_mode == 1) {
-          const long long off =
-              ((((long long)(m1 >> 3) * prm.nbv + (m2 >> 3)) * prm.nbv + (n >> 3)) << 9) +
-              ((((m1 & 7) << 3) + (m2 & 7)) << 3) + (n & 7);
-          if (has1) {
-            *reinterpret_cast<double2*>(C + off) = make_double2(acc[i][j][0], acc[i][j][1]);
-          } else {
-            C[off] = acc[i][j][0];
-          }
-        } else {
-          const long long base = (long long)m1 * prm.sM1 + (long long)m2 * prm.sM2;
-          const long long off0 = base + (long long)(n / prm.n2_ext) * prm.sN1 + (long long)(n % prm.n2_ext) * prm.sN2;
-          const long long off1 = base + (long long)((n + 1) / prm.n2_ext) * prm.sN1 +
-                                 (long long)((n + 1) % prm.n2_ext) * prm.sN2;
-          if (has1 && off1 == off0 + 1 && ((reinterpret_cast<uintptr_t>(C + off0) & 15) == 0)) {
-            *reinterpret_cast<double2*>(C + off0) = make_double2(acc[i][j][0], acc[i][j][1]);
-          } else {
-            C[off0] = acc[i][j][0];
-            if (has1) C[off1] = acc[i][j][1];
-          }
-        }
-      }
-    }
+  // warps w and w+4 share an SM sub-partition: they take the same rows and the two column halves, so that every
+  // sub-partition issues NF0 + NF1 fragments per k-step also when NF is odd.  The fragment count is a template
+  // argument of the consumer loop: no predicates in the DMMA sequence.
+  if constexpr (NF0 == NF1) {
+    gemm_consume<NF, NF0>(prm, smem, full_bar, empty_bar, warp, lane, (warp >> 2) * (8 * NF0), total_tiles,
+                          tiles_per_task, tq);
+  } else {
+    if ((warp >> 2) == 0)
+      gemm_consume<NF, NF0>(prm, smem, full_bar, empty_bar, warp, lane, 0, total_tiles, tiles_per_task, tq);
+    else
+      gemm_consume<NF, NF1>(prm, smem, full_bar, empty_bar, warp, lane, 8 * NF0, total_tiles, tiles_per_task, tq);
   }
 }
 
@@ -274,13 +302,13 @@ int make_tensor_map_f64(CUtensorMap* out, const void* base, const unsigned long 
 // prm.tasks must stay valid until the kernel ran.
 int launch_gemm_nt(int nf, const CUtensorMap& tmA, const CUtensorMap& tmAT, const CUtensorMap& tmB,
                    const GemmParams& prm, cudaStream_t stream);
-// NF that minimises padded work for an N extent (ties -> larger tile).
+// NF that minimises the modelled time (padded columns x per-tile efficiency) of an N extent.
 int choose_nf(long long n_ext);
-// Cover [0, n_ext) with the fewest column tiles of 16*NF, NF in [kMinNF, kMaxNF], spreading the slack evenly
-// so that the padded extent is n_ext rounded up to 16 whenever n_ext >= 16*kMinNF.  At most two distinct NF
+// Cover [0, n_ext) with the fewest column tiles of 8*NF, NF in [kMinNF, kMaxNF], spreading the slack evenly
+// so that the padded extent is n_ext rounded up to 8 whenever n_ext >= 8*kMinNF.  At most two distinct NF
 // values result; tiles of equal NF are adjacent.  Returns the number of segments written (<= 2).
 struct NSegment { int n0, ntiles, nf; };
-int split_n(int n_ext, NSegment seg[2]);
+int split_n(int n_ext, NSegment seg[2], int granularity = 8);   // granularity 16: even NF only
 // (tp, tq_log2) with tp * tq = 128 minimising padded rows for extents (m1_ext, m2_ext).
 void choose_m_tile(int m1_ext, int m2_ext, int* tp, int* tq_log2);
 

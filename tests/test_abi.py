@@ -107,18 +107,18 @@ def test_plan_and_workspace(libpath):
 
 def test_w_builder_tiling_covers_every_extent_exactly_once(libpath):
     """split_n / split_m: segments are disjoint, ordered, cover [0, v) and pad as little as
-    the tile shapes allow: N to the next multiple of 16 (>= 64), M rows to v (main) + a strip < one tile."""
+    the tile shapes allow: N to the next multiple of 8 (>= 32), M rows to v (main) + a strip < one tile."""
     import paper_2502_17963_b200 as bqc
     for v in list(range(1, 420)) + [512, 777, 1320]:
         cols, rows = bqc.bqc_debug_tiling(v)
         assert 1 <= len(cols) <= 2 and 1 <= len(rows) <= 2
-        # columns: contiguous segments, NF in [4, 8]
+        # columns: contiguous segments of tiles 8*NF wide, NF in [4, 16]
         n = 0
         for (n0, ntiles, nf) in cols:
-            assert n0 == n and ntiles >= 1 and 4 <= nf <= 8
-            n += ntiles * 16 * nf
-        assert n >= v and n == max(64, (v + 15) // 16 * 16)
-        assert sum(c[1] for c in cols) == max(1, -(-((v + 15) // 16) // 8))      # fewest tiles
+            assert n0 == n and ntiles >= 1 and 4 <= nf <= 16
+            n += ntiles * 8 * nf
+        assert n >= v and n == max(32, (v + 7) // 8 * 8)
+        assert sum(c[1] for c in cols) == max(1, -(-((v + 7) // 8) // 16))       # fewest tiles
         # rows: contiguous m1 ranges, tp * tq = 128, tq >= 8
         m = 0
         for (m1_0, tiles_m1, tp, tq) in rows:
