@@ -249,8 +249,8 @@ def run_mp2(args):
 
 # ----------------------------------------------------------------------------- our arm
 # bytes per W-builder launch (4 triplets) from the one `ncu --set full` capture named in profiles/README.md:
-# 13.94 GB read + 5.24 GB written at config 5 (algorithmic: 5.27 GB of F writes + L2-shared operand reads)
-NCU_TRAFFIC_W_BUILDER = {5: 13.939768e9 + 5.243941e9}
+# 15.33 GB read + 5.25 GB written at config 5 (algorithmic: 5.27 GB of F writes + L2-shared operand reads)
+NCU_TRAFFIC_W_BUILDER = {5: 15.330726e9 + 5.248752e9}
 
 
 def main():
@@ -427,7 +427,7 @@ def main():
                          "flops_per_launch": flops_rank / max(prof["gemm_launches"], 1),
                          "traffic": None if abc else NCU_TRAFFIC_W_BUILDER.get(args.config),
                          "traffic_source": "ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch "
-                                           "(profiles/r1b_gemm_nt_full.txt)" if (args.config in NCU_TRAFFIC_W_BUILDER
+                                           "(profiles/r1c_gemm_nt_full.txt)" if (args.config in NCU_TRAFFIC_W_BUILDER
                                                                                    and not abc)
                                            else None},
             "clocks": clocks,
