@@ -191,6 +191,8 @@ def run_mp2(args):
     host = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (inp.eps_occ, inp.eps_vir, inp.B_ov)]
     dev = [t.cuda() for t in host]
     opts = bqc.make_mp2_opts(occ_block=args.occ_block, flags=bqc.BQC_T_FLAG_PROFILE)
+    mp2_ws = torch.empty(bqc.bqc_mp2_workspace_bytes(o, v, X, opts), dtype=torch.uint8, device="cuda")
+    opts = bqc.make_mp2_opts(occ_block=args.occ_block, flags=bqc.BQC_T_FLAG_PROFILE, workspace=mp2_ws)
     peak = bqc.bqc_fp64_peak_tflops(0, args.peak_seconds)
     e_pair = torch.zeros((o, o), dtype=torch.float64, device="cuda")
     for _ in range(args.warmup):

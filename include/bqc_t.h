@@ -203,6 +203,8 @@ typedef struct bqc_mp2_opts {
   int shard_rank;    /* multi-GPU sharding: this call evaluates the occupied blocks whose number     */
   int shard_count;   /*   % shard_count == shard_rank (all pairs i <= j of those rows i).  0 -> 1.  */
   int flags;         /* BQC_T_FLAG_PROFILE: time the kernel groups, read with bqc_mp2_last_profile  */
+  void* workspace;   /* optional caller-owned DEVICE scratch, 256-byte aligned, >= bqc_mp2_workspace_bytes; */
+  size_t workspace_bytes; /* NULL / 0: one block is allocated internally and freed before return      */
 } bqc_mp2_opts;
 
 /* E_MP2 in Hartree; NaN on error.  DEVICE pointers: eps_occ [nocc], eps_vir [nvir],
@@ -229,6 +231,8 @@ BQC_API int bqc_mp2_energy_host(int nocc, int nvir, int naux, const double* eps_
 /* Algorithmic FP64 flop count of the (ov|ov) contraction over the pairs i <= j:
    o(o+1)/2 * 2 v^2 X (the energy reduction, ~8 flops per element, is not counted). */
 BQC_API double bqc_mp2_flops(int nocc, int nvir, int naux);
+/* Bytes of device scratch bqc_mp2_energy_ex needs for these sizes/options (0 on bad arguments). */
+BQC_API size_t bqc_mp2_workspace_bytes(int nocc, int nvir, int naux, const bqc_mp2_opts* opts);
 /* Occupied block size bqc_mp2_energy_ex will use (resolves opts->occ_block == 0); -1 on bad sizes. */
 BQC_API int bqc_mp2_plan_occ_block(int nocc, int nvir, int naux, const bqc_mp2_opts* opts);
 /* Timing of this thread's last profiled bqc_mp2_energy_ex call (CUDA events on the launch stream):

@@ -10,7 +10,7 @@ from .binding import (BQC_T_FLAG_NO_T1, BQC_T_FLAG_PROFILE, BQC_T_FLAG_ABC_DRIVE
                       bqc_t_num_triplets, bqc_t_opts, bqc_t_plan_occ_block, bqc_t_triplet_index,
                       bqc_t_triplet_owner, bqc_t_workspace_bytes, bqc_version, lib, make_opts,
                       bqc_mp2_energy, bqc_mp2_energy_ex, bqc_mp2_energy_host, bqc_mp2_flops, bqc_mp2_last_profile,
-                      bqc_mp2_opts, bqc_mp2_plan_occ_block, make_mp2_opts)
+                      bqc_mp2_opts, bqc_mp2_plan_occ_block, bqc_mp2_workspace_bytes, make_mp2_opts)
 
 from .distributed import bqc_t_energy_sharded, combine_partials
 

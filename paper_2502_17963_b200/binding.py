@@ -30,7 +30,8 @@ class bqc_t_opts(Structure):
 
 
 class bqc_mp2_opts(Structure):
-    _fields_ = [("occ_block", c_int), ("shard_rank", c_int), ("shard_count", c_int), ("flags", c_int)]
+    _fields_ = [("occ_block", c_int), ("shard_rank", c_int), ("shard_count", c_int), ("flags", c_int),
+                ("workspace", c_void_p), ("workspace_bytes", c_size_t)]
 
 
 BQC_T_FLAG_NO_T1 = 1
@@ -54,6 +55,8 @@ def lib():
     L.bqc_t_num_triplets.argtypes = [c_int]
     L.bqc_t_triplet_index.restype = c_size_t
     L.bqc_t_triplet_index.argtypes = [c_int] * 4
+    L.bqc_mp2_workspace_bytes.restype = c_size_t
+    L.bqc_mp2_workspace_bytes.argtypes = [c_int] * 3 + [POINTER(bqc_mp2_opts)]
     L.bqc_debug_tiling.restype = c_int
     L.bqc_debug_tiling.argtypes = [c_int, POINTER(c_int), c_int]
     L.bqc_t_triplet_owner.restype = c_int
@@ -255,8 +258,17 @@ def bqc_t_energy_host(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_
 
 
 # ---------------------------------------------------------------- DF-MP2 energy (Eq. (1))
-def make_mp2_opts(occ_block=0, shard_rank=0, shard_count=1, flags=0):
-    return bqc_mp2_opts(occ_block, shard_rank, shard_count, flags)
+def make_mp2_opts(occ_block=0, shard_rank=0, shard_count=1, flags=0, workspace=None):
+    """`workspace`: optional uint8 CUDA tensor of >= bqc_mp2_workspace_bytes (kept alive by the caller)."""
+    o = bqc_mp2_opts(occ_block, shard_rank, shard_count, flags, None, 0)
+    if workspace is not None:
+        o.workspace = workspace.data_ptr()
+        o.workspace_bytes = workspace.numel() * workspace.element_size()
+    return o
+
+
+def bqc_mp2_workspace_bytes(nocc, nvir, naux, opts=None):
+    return lib().bqc_mp2_workspace_bytes(nocc, nvir, naux, _optp(opts))
 
 
 def _mp2_inputs(nocc, nvir, naux, eps_occ, eps_vir, B_ov, device):

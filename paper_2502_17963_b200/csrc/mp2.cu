@@ -133,6 +133,27 @@ int resolve_block(int o, int v, const bqc_mp2_opts* opts, int* bi) {
   return BQC_OK;
 }
 
+struct Mp2Layout {
+  size_t off_bt = 0, off_jblk = 0, off_partial = 0, off_epair = 0, off_ew = 0, off_esum = 0, off_tiles = 0,
+         off_task = 0, total = 0;
+};
+
+Mp2Layout mp2_layout(int o, int v, int Xp, int Bi, int ntp) {
+  Mp2Layout L;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t r = off; off = round_up(off + (bytes ? bytes : 8), 1024); return r; };
+  L.off_bt = take((size_t)o * v * Xp * 8);                    // Bt_ov
+  L.off_jblk = take((size_t)Bi * v * ((size_t)o * v) * 8);    // (ov|ov) block
+  L.off_partial = take((size_t)Bi * o * ntp * 8);
+  L.off_epair = take((size_t)o * o * 8);
+  L.off_ew = take((size_t)o * o * 8);
+  L.off_esum = take(64);
+  L.off_tiles = take((size_t)ntp * 4);
+  L.off_task = take(sizeof(GemmTask));
+  L.total = off;
+  return L;
+}
+
 struct Scratch {
   std::vector<void*> ptrs;
   std::vector<cudaEvent_t> evs;
@@ -201,17 +222,28 @@ static int mp2_impl(int o, int v, int X, const double* eps_occ, const double* ep
   const int nt = ceil_div(v, kMT), ntp = nt * (nt + 1) / 2;
   const long long ld_max = (long long)o * v;
   Scratch sc_mem;
-  double *bt = nullptr, *jblk = nullptr, *partial = nullptr, *e_pair = nullptr, *e_w = nullptr, *e_sum = nullptr;
-  int* tiles = nullptr;
-  GemmTask* task_dev = nullptr;
-  BQC_TRY(sc_mem.alloc((void**)&bt, (size_t)o * v * Xp * 8, "Bt_ov"));
-  BQC_TRY(sc_mem.alloc((void**)&jblk, (size_t)Bi * v * ld_max * 8, "(ov|ov) block"));
-  BQC_TRY(sc_mem.alloc((void**)&partial, (size_t)Bi * o * ntp * 8, "partials"));
-  BQC_TRY(sc_mem.alloc((void**)&e_pair, (size_t)o * o * 8, "e_pair"));
-  BQC_TRY(sc_mem.alloc((void**)&e_w, (size_t)o * o * 8, "e_w"));
-  BQC_TRY(sc_mem.alloc((void**)&e_sum, 64, "e_sum"));
-  BQC_TRY(sc_mem.alloc((void**)&tiles, (size_t)ntp * 4, "tile table"));
-  BQC_TRY(sc_mem.alloc((void**)&task_dev, sizeof(GemmTask), "task"));
+  // one workspace block: the caller's (opts->workspace) or one cudaMalloc freed before return
+  const Mp2Layout L = mp2_layout(o, v, Xp, Bi, ntp);
+  uint8_t* ws = nullptr;
+  if (opts && opts->workspace) {
+    if (opts->workspace_bytes < L.total || (reinterpret_cast<uintptr_t>(opts->workspace) & 255)) {
+      set_error(BQC_ERR_WORKSPACE, "mp2 workspace of %zu bytes (need %zu, 256-byte aligned)", opts->workspace_bytes,
+                L.total);
+      return BQC_ERR_WORKSPACE;
+    }
+    BQC_TRY(check_device_ptr(opts->workspace, "opts->workspace"));
+    ws = static_cast<uint8_t*>(opts->workspace);
+  } else {
+    BQC_TRY(sc_mem.alloc((void**)&ws, L.total, "mp2 workspace"));
+  }
+  double* bt = reinterpret_cast<double*>(ws + L.off_bt);
+  double* jblk = reinterpret_cast<double*>(ws + L.off_jblk);
+  double* partial = reinterpret_cast<double*>(ws + L.off_partial);
+  double* e_pair = reinterpret_cast<double*>(ws + L.off_epair);
+  double* e_w = reinterpret_cast<double*>(ws + L.off_ew);
+  double* e_sum = reinterpret_cast<double*>(ws + L.off_esum);
+  int* tiles = reinterpret_cast<int*>(ws + L.off_tiles);
+  GemmTask* task_dev = reinterpret_cast<GemmTask*>(ws + L.off_task);
 
   int nlaunch = 0;
   if (prof) BQC_TRY(sc_mem.mark(s));   // evs[0]: begin
@@ -317,6 +349,15 @@ extern "C" {
 double bqc_mp2_flops(int nocc, int nvir, int naux) {
   if (nocc <= 0 || nvir <= 0 || naux <= 0) return 0.0;
   return 0.5 * nocc * (nocc + 1.0) * 2.0 * (double)nvir * nvir * naux;
+}
+
+size_t bqc_mp2_workspace_bytes(int nocc, int nvir, int naux, const bqc_mp2_opts* opts) {
+  clear_error();
+  if (check_sizes(nocc, nvir, naux) != BQC_OK) return 0;
+  int bi = 0;
+  if (resolve_block(nocc, nvir, opts, &bi) != BQC_OK) return 0;
+  const int nt = ceil_div(nvir, kMT);
+  return mp2_layout(nocc, nvir, round_up_i(naux, 16), bi, nt * (nt + 1) / 2).total;
 }
 
 int bqc_mp2_plan_occ_block(int nocc, int nvir, int naux, const bqc_mp2_opts* opts) {

@@ -88,6 +88,14 @@ def test_mp2_host_entry_point_and_errors():
     assert ei.value.code == 8                        # BQC_ERR_DENOMINATOR
     with pytest.raises(bqc.BqcError):
         bqc.bqc_mp2_energy_ex(o, v, X, *d, opts=bqc.make_mp2_opts(shard_rank=3, shard_count=2))
+    # caller workspace: same bits as the internally allocated one; too small is refused
+    e_dev = bqc.bqc_mp2_energy_ex(o, v, X, *d)
+    need = bqc.bqc_mp2_workspace_bytes(o, v, X)
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    assert bqc.bqc_mp2_energy_ex(o, v, X, *d, opts=bqc.make_mp2_opts(workspace=ws)) == e_dev == e
+    with pytest.raises(bqc.BqcError) as ei:
+        bqc.bqc_mp2_energy_ex(o, v, X, *d, opts=bqc.make_mp2_opts(workspace=ws[: need - 1024]))
+    assert ei.value.code == 5                        # BQC_ERR_WORKSPACE
 
 
 def test_mp2_config3_sampled_pairs():
