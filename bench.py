@@ -290,7 +290,8 @@ def main():
     lo = 0 if args.full else (rank % nblocks) * w
     hi = nidx if args.full else lo + w
     if args.full and world > 1:
-        opts = bqc.make_opts(occ_block=args.occ_block, shard_rank=rank, shard_count=world, flags=sched_flags)
+        opts = bqc.make_opts(occ_block=args.occ_block, shard_rank=rank, shard_count=world,
+                             flags=sched_flags | bqc.BQC_T_FLAG_SHARD_BLOCKS)
     else:
         opts = bqc.make_opts(occ_block=args.occ_block, occ_lo=lo, occ_hi=hi, flags=sched_flags)
     flops_rank = bqc.bqc_t_flops(o, v, opts)
@@ -369,7 +370,7 @@ def main():
         torch.cuda.empty_cache()
         eopts = bqc.make_opts(occ_block=args.occ_block, occ_lo=opts.occ_lo, occ_hi=opts.occ_hi,
                               shard_rank=opts.shard_rank, shard_count=opts.shard_count,
-                              flags=bqc.BQC_T_FLAG_ABC_DRIVEN if abc else 0)
+                              flags=opts.flags & ~bqc.BQC_T_FLAG_PROFILE)
         barrier()
         t0 = time.perf_counter()
         for _ in range(args.e2e_steps):

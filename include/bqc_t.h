@@ -92,7 +92,15 @@ enum {
                                    per-virtual-triple contributions (2 - d_ab - d_bc) sum_ijk R V / D, and
                                    bqc_t_flops counts 12 o^3 (v+o) per virtual triple.  The library builds
                                    the transposed amplitude / DF arrays it needs inside the workspace
-                                   (one extra copy of t2 and B_ov).                                      */
+                                   (one extra copy of t2 and B_ov).                                      */,
+  BQC_T_FLAG_SHARD_BLOCKS = 8   /* multi-GPU sharding by whole block triples instead of single triplets: with
+                                   shard_count > 1 this call evaluates the block triples (I <= J <= K blocks
+                                   of occ_block orbitals, numbered in loop order) whose number % shard_count
+                                   == shard_rank, and forms only the (vv|ov) slabs those need — the per-triplet
+                                   modulo makes every shard form every slab.  Shards are still disjoint and
+                                   cover every triplet once; per-triplet values are the same bits.  The split
+                                   depends on occ_block (bqc_t_plan_occ_block); bqc_t_triplet_owner does not
+                                   describe it.                                                        */
 };
 
 /* ---- host-only helpers (no GPU needed) -------------------------------------------------- */

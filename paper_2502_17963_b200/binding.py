@@ -37,6 +37,7 @@ class bqc_mp2_opts(Structure):
 BQC_T_FLAG_NO_T1 = 1
 BQC_T_FLAG_PROFILE = 2
 BQC_T_FLAG_ABC_DRIVEN = 4
+BQC_T_FLAG_SHARD_BLOCKS = 8
 
 _lib = None
 

@@ -27,6 +27,7 @@ namespace {
 
 constexpr int kMT = 32;            // tile edge of the pair-energy kernel
 constexpr int kMThreads = 256;     // 32 x 8 threads, 4 tile rows each
+constexpr int kGemmRows = 2;       // occupied rows per (ov|ov) GEMM sub-launch
 
 static thread_local double g_mp2_profile[6] = {0, 0, 0, 0, 0, 0};
 
@@ -268,13 +269,18 @@ static int mp2_impl(int o, int v, int X, const double* eps_occ, const double* ep
   for (int b = 0; b < nblk; ++b) {
     if (b % sc != sr) continue;
     const int i0 = b * Bi, i1 = std::min(o, i0 + Bi);
-    const int M = (i1 - i0) * v;
-    const long long N = (long long)(o - i0) * v;
-    const long long ld = N;
-    const int nf = choose_nf(N);
-    CUtensorMap tA, tB;
-    const double* base = bt + (size_t)i0 * v * Xp;   // rows (i0, 0) onwards; 128-byte aligned (Xp % 16 == 0)
-    {
+    const long long ld = (long long)(o - i0) * v;
+    // The (ov|ov) rows of the block are formed kGemmRows occupied orbitals at a time, each sub-launch covering
+    // only the columns j >= its first row: the pairs j < i that a rectangular block GEMM would also compute
+    // shrink from ~15 % of the work (18-row blocks at config 5) to ~1.5 %.
+    if (prof) BQC_TRY(sc_mem.mark(s));
+    for (int g0 = i0; g0 < i1; g0 += kGemmRows) {
+      const int g1 = std::min(i1, g0 + kGemmRows);
+      const int M = (g1 - g0) * v;
+      const long long N = (long long)(o - g0) * v;
+      const int nf = choose_nf(N);
+      CUtensorMap tA, tB;
+      const double* base = bt + (size_t)g0 * v * Xp;   // rows (g0, 0) onwards; 128-byte aligned (Xp % 16 == 0)
       const unsigned long long dA[4] = {(unsigned long long)Xp, (unsigned long long)M, 1, 1};
       const unsigned long long sA[4] = {8, (unsigned long long)Xp * 8, (unsigned long long)Xp * 8 * M,
                                         (unsigned long long)Xp * 8 * M};
@@ -283,23 +289,24 @@ static int mp2_impl(int o, int v, int X, const double* eps_occ, const double* ep
       const unsigned long long sB[4] = {8, (unsigned long long)Xp * 8, (unsigned long long)Xp * 8 * N,
                                         (unsigned long long)Xp * 8 * N};
       BQC_TRY(make_tensor_map_f64(&tB, base, dB, sB, gemm_bn(nf), 1));
+      GemmParams prm;
+      memset(&prm, 0, sizeof(prm));
+      prm.ntasks = 1;
+      prm.tp = 1; prm.tq_log2 = 7;
+      prm.tiles_m1 = 1;
+      prm.tiles_m2 = ceil_div(M, kBM);
+      prm.tiles_n = (int)((N + gemm_bn(nf) - 1) / gemm_bn(nf));
+      prm.m1_ext = 1; prm.m2_ext = M; prm.n_ext = (int)N;
+      prm.kiters = Xp / kBK;
+      prm.out_mode = 0;
+      prm.n2_ext = INT_MAX;
+      prm.sM1 = 0; prm.sM2 = ld; prm.sN1 = 0; prm.sN2 = 1;
+      prm.tasks = task_dev;
+      // element (row (i - g0) v + a, column (j - g0) v + b) of this sub-launch -> Jblk[(i - i0) v + a][(j - i0) v + b]
+      prm.C = jblk + (long long)(g0 - i0) * v * ld + (long long)(g0 - i0) * v;
+      BQC_TRY(launch_gemm_nt(nf, tA, tA, tB, prm, s));
+      ++nlaunch;
     }
-    GemmParams prm;
-    memset(&prm, 0, sizeof(prm));
-    prm.ntasks = 1;
-    prm.tp = 1; prm.tq_log2 = 7;
-    prm.tiles_m1 = 1;
-    prm.tiles_m2 = ceil_div(M, kBM);
-    prm.tiles_n = (int)((N + gemm_bn(nf) - 1) / gemm_bn(nf));
-    prm.m1_ext = 1; prm.m2_ext = M; prm.n_ext = (int)N;
-    prm.kiters = Xp / kBK;
-    prm.out_mode = 0;
-    prm.n2_ext = INT_MAX;
-    prm.sM1 = 0; prm.sM2 = ld; prm.sN1 = 0; prm.sN2 = 1;
-    prm.tasks = task_dev;
-    prm.C = jblk;
-    if (prof) BQC_TRY(sc_mem.mark(s));
-    BQC_TRY(launch_gemm_nt(nf, tA, tA, tB, prm, s));
     if (prof) BQC_TRY(sc_mem.mark(s));
     ++ngemm;
 
@@ -314,7 +321,7 @@ static int mp2_impl(int o, int v, int X, const double* eps_occ, const double* ep
     count_launch();
     BQC_CUDA_OK(cudaGetLastError());
     if (prof) BQC_TRY(sc_mem.mark(s));
-    nlaunch += 3;
+    nlaunch += 2;
   }
   BQC_TRY(launch_final_sum(e_w, (long long)o * o, e_sum, s));
   ++nlaunch;

@@ -58,6 +58,7 @@ struct Plan {
   int use_t1 = 1;
   int profile = 0;
   int shard_rank = 0, shard_count = 1;
+  int shard_blocks = 0;        // BQC_T_FLAG_SHARD_BLOCKS
   // workspace offsets (bytes)
   size_t off_btvv = 0, off_btov = 0, off_btoo = 0, off_btil = 0, off_J = 0, off_slabs = 0, off_F = 0,
          off_partial = 0, off_etrip = 0, off_esum = 0, off_act = 0, off_orbits = 0, off_tasks = 0,
@@ -116,6 +117,7 @@ int make_plan(Plan& P, int o, int v, int X, const std::vector<int>& act, const b
   P.profile = (opts && (opts->flags & BQC_T_FLAG_PROFILE)) ? 1 : 0;
   P.shard_count = (opts && opts->shard_count > 0) ? opts->shard_count : 1;
   P.shard_rank = opts ? opts->shard_rank : 0;
+  P.shard_blocks = (opts && (opts->flags & BQC_T_FLAG_SHARD_BLOCKS)) ? 1 : 0;
   if (P.shard_rank < 0 || P.shard_rank >= P.shard_count) {
     set_error(BQC_ERR_INVALID_OPTION, "shard_rank %d outside [0,%d)", P.shard_rank, P.shard_count);
     return BQC_ERR_INVALID_OPTION;
@@ -575,17 +577,17 @@ int Pipeline::build_schedule() {
   };
   auto slot_of = [&](int pos, int set, int block) { return set * P.Bo + (pos - block_begin(block)); };
 
+  long long block_triple = -1;
   for (int I = 0; I < P.nblk; ++I) {
-    acquire(0, I);
     for (int Jb = I; Jb < P.nblk; ++Jb) {
       const int sJ = (Jb == I) ? 0 : 1;
-      if (Jb != I) acquire(1, Jb);
       for (int K = Jb; K < P.nblk; ++K) {
+        ++block_triple;
+        // BQC_T_FLAG_SHARD_BLOCKS: whole block triples are dealt to the shards, so a shard forms only the
+        // slabs of its own block triples; otherwise every shard owns some triplets of every block triple
+        if (P.shard_blocks && (int)(block_triple % P.shard_count) != P.shard_rank) continue;
         int sK = sJ;
-        if (K != Jb) {
-          sK = 2 + (kflip++ & 1);
-          acquire(sK, K);
-        }
+        if (K != Jb) sK = (set_block[2] == K) ? 2 : (set_block[3] == K ? 3 : 2 + (kflip++ & 1));
         // triplets of this block triple owned by this shard
         std::vector<TripletRec> list;
         std::vector<int> slots;   // 3 per triplet
@@ -597,12 +599,17 @@ int Pipeline::build_schedule() {
               t.i = P.act[pi]; t.j = P.act[pj]; t.k = P.act[pk];
               t.pi = pi; t.pj = pj; t.pk = pk;
               t.index = (long long)triplet_index(P.o, t.i, t.j, t.k);
-              if ((int)(t.index % P.shard_count) != P.shard_rank) continue;
+              if (!P.shard_blocks && (int)(t.index % P.shard_count) != P.shard_rank) continue;
               list.push_back(t);
               slots.push_back(slot_of(pi, 0, I));
               slots.push_back(slot_of(pj, sJ, Jb));
               slots.push_back(slot_of(pk, sK, K));
             }
+        if (list.empty()) continue;
+        // slabs are formed only for block triples that have work (the acquire calls are idempotent)
+        acquire(0, I);
+        if (Jb != I) acquire(1, Jb);
+        if (K != Jb) acquire(sK, K);
         for (size_t b0 = 0; b0 < list.size(); b0 += P.nbatch) {
           const size_t nb = std::min(list.size() - b0, (size_t)P.nbatch);
           Action a;
@@ -918,6 +925,27 @@ double bqc_t_flops(int nocc, int nvir, const bqc_t_opts* opts) {
   const int sc = (opts && opts->shard_count > 0) ? opts->shard_count : 1;
   const int sr = opts ? opts->shard_rank : 0;
   size_t n = 0;
+  if (opts && (opts->flags & BQC_T_FLAG_SHARD_BLOCKS) && sc > 1) {
+    // same block-triple walk as Pipeline::build_schedule (the block size does not depend on naux)
+    Plan P;
+    std::vector<int> act(hi - lo);
+    for (int x = lo; x < hi; ++x) act[x - lo] = x;
+    if (make_plan(P, nocc, nvir, 1, act, opts) != BQC_OK) return -1.0;
+    auto b0 = [&](int b) { return b * P.Bo; };
+    auto b1 = [&](int b) { return std::min(P.na, (b + 1) * P.Bo); };
+    long long bt = -1;
+    for (int I = 0; I < P.nblk; ++I)
+      for (int J = I; J < P.nblk; ++J)
+        for (int K = J; K < P.nblk; ++K) {
+          if ((int)(++bt % sc) != sr) continue;
+          for (int pi = b0(I); pi < b1(I); ++pi)
+            for (int pj = std::max(pi, b0(J)); pj < b1(J); ++pj)
+              for (int pk = std::max(pj, b0(K)); pk < b1(K); ++pk)
+                if (!(pi == pj && pj == pk)) ++n;
+        }
+    const double v = nvir;
+    return (double)n * 12.0 * v * v * v * (v + nocc);
+  }
   for (int i = lo; i < hi; ++i)
     for (int j = i; j < hi; ++j)
       for (int k = j; k < hi; ++k) {

@@ -1,7 +1,8 @@
 """One process per GPU: triplet sharding + the path's single exchange.
 
-Triplets are independent, so each rank evaluates the triplets `bqc_t_triplet_index % world == rank`
-(`bqc_t_opts.shard_rank / shard_count`) on its own replica of the inputs and there is no data-path
+Triplets are independent, so each rank evaluates its share of them (`bqc_t_opts.shard_rank /
+shard_count`; by default whole block triples, `BQC_T_FLAG_SHARD_BLOCKS`, so that a rank forms only the
+(vv|ov) slabs its own triplets need) on its own replica of the inputs and there is no data-path
 collective.  The only exchange is the final scalar: the per-rank partial sums are all-gathered and
 added in rank order, so every rank returns the same bits and the result does not depend on arrival
 order (an 8-byte all-reduce would do when that is not required).  Argument marshalling and
@@ -40,7 +41,8 @@ def bqc_t_energy_sharded(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov,
     """
     rank = dist.get_rank(group) if dist.is_initialized() else 0
     world = dist.get_world_size(group) if dist.is_initialized() else 1
-    opts = _b.make_opts(occ_block=occ_block, shard_rank=rank, shard_count=world, flags=flags, f_ov=f_ov)
+    opts = _b.make_opts(occ_block=occ_block, shard_rank=rank, shard_count=world,
+                        flags=flags | _b.BQC_T_FLAG_SHARD_BLOCKS, f_ov=f_ov)
     e_local = _b.bqc_t_energy_ex(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, opts=opts,
                                  workspace=workspace, e_triplet=e_triplet)
     return combine_partials(e_local, group)

@@ -130,3 +130,17 @@ def test_w_builder_tiling_covers_every_extent_exactly_once(libpath):
         padded = sum(t * tp * (-(-v // tq) * tq) for (_, t, tp, tq) in rows)
         single = min(-(-v // (128 // tq)) * (128 // tq) * (-(-v // tq) * tq) for tq in (8, 16, 32, 64, 128))
         assert padded <= single                                        # never worse than one tile shape
+
+
+def test_block_triple_sharding_flop_model_partitions_the_work(libpath):
+    import paper_2502_17963_b200 as bqc
+    F = bqc.BQC_T_FLAG_SHARD_BLOCKS
+    for (o, v, bo) in [(20, 76, 0), (100, 380, 0), (100, 380, 5), (7, 11, 2)]:
+        total = bqc.bqc_t_flops(o, v)
+        for world in (1, 2, 8):
+            parts = [bqc.bqc_t_flops(o, v, bqc.make_opts(shard_rank=r, shard_count=world, occ_block=bo, flags=F))
+                     for r in range(world)]
+            assert sum(parts) == total
+    # config 5, 8 shards: within a few per cent of an even split
+    parts = [bqc.bqc_t_flops(100, 380, bqc.make_opts(shard_rank=r, shard_count=8, flags=F)) for r in range(8)]
+    assert max(parts) / (sum(parts) / 8) < 1.05

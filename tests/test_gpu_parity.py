@@ -214,6 +214,41 @@ def test_blocking_window_and_sharding_agree_bitwise():
     assert abs(ew - ref) <= e_tol(ref)
 
 
+def test_block_triple_sharding_is_disjoint_bitwise_and_forms_fewer_slabs():
+    """BQC_T_FLAG_SHARD_BLOCKS: whole block triples per shard."""
+    inp = make_inputs(9, 19, 13, seed=53, t1_std=0.05)
+    d = to_device(inp)
+    o = inp.nocc
+    n = bqc.bqc_t_num_triplets(o)
+    base = torch.empty(n, dtype=torch.float64, device="cuda")
+    e_all = bqc.bqc_t_energy_ex(*dims(inp), *d, opts=bqc.make_opts(occ_block=2, flags=bqc.BQC_T_FLAG_PROFILE),
+                                e_triplet=base)
+    forms_all = bqc.bqc_t_last_profile()["form_blocks"]
+    F = bqc.BQC_T_FLAG_SHARD_BLOCKS | bqc.BQC_T_FLAG_PROFILE
+    for world in (2, 3, 5):
+        parts, flops, forms, es = [], 0.0, [], []
+        for r in range(world):
+            et = torch.empty_like(base)
+            opts = bqc.make_opts(shard_rank=r, shard_count=world, occ_block=2, flags=F)
+            es.append(bqc.bqc_t_energy_ex(*dims(inp), *d, opts=opts, e_triplet=et))
+            forms.append(bqc.bqc_t_last_profile()["form_blocks"])
+            flops += bqc.bqc_t_flops(o, inp.nvir, opts)
+            # the flop model counts exactly the triplets this shard evaluated
+            nz = int((et != 0).sum())
+            assert bqc.bqc_t_flops(o, inp.nvir, opts) == nz * 12.0 * inp.nvir ** 3 * (inp.nvir + o)
+            parts.append(et)
+        assert torch.equal(sum(parts), base)                                # same bits, every triplet once
+        for idx in range(n):
+            assert sum(int(p[idx] != 0) for p in parts) <= 1
+        assert flops == bqc.bqc_t_flops(o, inp.nvir)
+        assert abs(sum(es) - e_all) <= e_tol(e_all)
+        assert max(forms) < forms_all                                       # a shard forms only what it needs
+    # one shard: the flag changes nothing
+    et = torch.empty_like(base)
+    bqc.bqc_t_energy_ex(*dims(inp), *d, opts=bqc.make_opts(occ_block=2, flags=bqc.BQC_T_FLAG_SHARD_BLOCKS), e_triplet=et)
+    assert torch.equal(et, base)
+
+
 def test_deterministic_and_workspace_and_host_paths():
     inp = make_config(1, t1_std=0.01)
     d = to_device(inp)
