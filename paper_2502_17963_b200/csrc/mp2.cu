@@ -27,7 +27,6 @@ namespace {
 
 constexpr int kMT = 32;            // tile edge of the pair-energy kernel
 constexpr int kMThreads = 256;     // 32 x 8 threads, 4 tile rows each
-constexpr int kGemmRows = 2;       // occupied rows per (ov|ov) GEMM sub-launch
 
 static thread_local double g_mp2_profile[6] = {0, 0, 0, 0, 0, 0};
 
@@ -270,12 +269,13 @@ static int mp2_impl(int o, int v, int X, const double* eps_occ, const double* ep
     if (b % sc != sr) continue;
     const int i0 = b * Bi, i1 = std::min(o, i0 + Bi);
     const long long ld = (long long)(o - i0) * v;
-    // The (ov|ov) rows of the block are formed kGemmRows occupied orbitals at a time, each sub-launch covering
-    // only the columns j >= its first row: the pairs j < i that a rectangular block GEMM would also compute
-    // shrink from ~15 % of the work (18-row blocks at config 5) to ~1.5 %.
+    // The (ov|ov) rows of the block are formed `grows` occupied orbitals at a time, each sub-launch covering only
+    // the columns j >= its first row: the pairs j < i that a rectangular block GEMM would also compute shrink
+    // from ~15 % of the work (18-row blocks at config 5) to ~2 %.  grows keeps >= ~8 waves of tiles per launch.
+    const int grows = std::max(2, std::min(Bi, (int)ceil(3.9e7 / ((double)o * v * v))));
     if (prof) BQC_TRY(sc_mem.mark(s));
-    for (int g0 = i0; g0 < i1; g0 += kGemmRows) {
-      const int g1 = std::min(i1, g0 + kGemmRows);
+    for (int g0 = i0; g0 < i1; g0 += grows) {
+      const int g1 = std::min(i1, g0 + grows);
       const int M = (g1 - g0) * v;
       const long long N = (long long)(o - g0) * v;
       const int nf = choose_nf(N);
