@@ -99,6 +99,11 @@ def test_abc_driven_windows_blocks_and_shards_are_bitwise_consistent():
     assert np.array_equal(sum(parts), t_all)
     for n in range(len(t_all)):
         assert sum(1 for p in parts if p[n] != 0.0) <= 1
+    # whole block triples of virtuals per shard (BQC_T_FLAG_SHARD_BLOCKS): same bits, every triple once
+    parts = [_run(inp, shard_rank=r, shard_count=4, occ_block=5, flags=bqc.BQC_T_FLAG_SHARD_BLOCKS)[1] for r in range(4)]
+    assert np.array_equal(sum(parts), t_all)
+    for n in range(len(t_all)):
+        assert sum(1 for p in parts if p[n] != 0.0) <= 1
     # a virtual window [lo,hi): exactly the triples inside it
     lo, hi = 5, 14
     e_w, t_w = _run(inp, occ_lo=lo, occ_hi=hi)
