@@ -65,7 +65,8 @@ typedef struct bqc_t_opts {
   int occ_lo;        /* restrict to triplets with occ_lo <= i <= j <= k < occ_hi;            */
   int occ_hi;        /*   occ_lo = occ_hi = 0 means all occupied orbitals.                   */
   int shard_rank;    /* multi-GPU sharding: this call evaluates the triplets whose index     */
-  int shard_count;   /*   (bqc_t_triplet_index) % shard_count == shard_rank.  0 -> 1.        */
+  int shard_count;   /*   (bqc_t_triplet_index) % shard_count == shard_rank.  0 -> 1.
+                        (BQC_T_FLAG_SHARD_BLOCKS deals whole block triples instead.)         */
   int max_batch;     /* triplets per W-builder launch (0 = auto from memory)                 */
   int flags;         /* BQC_T_FLAG_* below                                                   */
   int reserved;
@@ -80,7 +81,7 @@ enum {
   BQC_T_FLAG_NO_T1 = 1,         /* drop the t1 (E[5]) and Fock terms: V = W (E[4]-only checks) */
   BQC_T_FLAG_PROFILE = 2,       /* bracket every kernel group with CUDA events on its launching
                                    stream; read the sums with bqc_t_last_profile             */
-  BQC_T_FLAG_ABC_DRIVEN = 4     /* abc-driven schedule (the paper's loop order; SURVEY.md
+  BQC_T_FLAG_ABC_DRIVEN = 4,    /* abc-driven schedule (the paper's loop order; SURVEY.md
                                    §8(f) NEXT-2): the outer loop runs over virtual triples a<=b<=c with all
                                    o^3 occupied triples inside, instead of occupied triplets i<=j<=k with
                                    all v^3 virtual triples inside.  Same E(T) up to summation order; the
@@ -92,7 +93,7 @@ enum {
                                    per-virtual-triple contributions (2 - d_ab - d_bc) sum_ijk R V / D, and
                                    bqc_t_flops counts 12 o^3 (v+o) per virtual triple.  The library builds
                                    the transposed amplitude / DF arrays it needs inside the workspace
-                                   (one extra copy of t2 and B_ov).                                      */,
+                                   (one extra copy of t2 and B_ov).                                      */
   BQC_T_FLAG_SHARD_BLOCKS = 8   /* multi-GPU sharding by whole block triples instead of single triplets: with
                                    shard_count > 1 this call evaluates the block triples (I <= J <= K blocks
                                    of occ_block orbitals, numbered in loop order) whose number % shard_count
