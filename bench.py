@@ -55,6 +55,11 @@ def parse():
     ap.add_argument("--peak-seconds", type=float, default=2.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-triplets", type=int, default=3, help="triplets the oracle evaluates (cpu_baseline)")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="torch.distributed backend of the N>1 plumbing (barrier, max-over-ranks, the scalar exchange)")
+    ap.add_argument("--share-gpu", action="store_true",
+                    help="TEST ONLY: every rank uses cuda:0 (implies --backend gloo); exercises the N>1 code path on a "
+                         "1-GPU box, its timings mean nothing and the line says so")
     ap.add_argument("--path", default="t", choices=["t", "mp2"],
                     help="t: the (T) energy (the headline); mp2: the DF-MP2 energy of PAPER.md Eq. (1) (SURVEY NEXT-4)")
     return ap.parse_args()
@@ -69,6 +74,42 @@ def workload_name(cfg, c, lo, hi, full, ntrip, abc=False):
     if full:
         return base + f", full E(T): all {ntrip} triplets i<=j<=k"
     return base + f", one triplet block per GPU: occupied window [{lo},{hi}) = {ntrip} triplets"
+
+
+# ----------------------------------------------------------------------------- one process per GPU
+def ensure_ranks(args):
+    """`python bench.py --gpus N` (no torchrun) starts the N ranks itself: it re-executes under
+    `python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1`, rank r bound to
+    GPU r.  Under torchrun (WORLD_SIZE set) it only checks that WORLD_SIZE matches --gpus."""
+    if args.gpus < 1:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} must be >= 1")
+    if args.share_gpu:
+        args.backend = "gloo"
+    world_env = os.environ.get("WORLD_SIZE")
+    if args.impl == "reference":
+        return                                  # the oracle arm runs on rank 0's host cores only
+    if world_env is not None:
+        if int(world_env) != args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world_env}; launch with "
+                             f"--nproc-per-node {args.gpus} or drop torchrun and let bench.py start the ranks")
+        return
+    if args.gpus == 1:
+        return
+    if args.path == "mp2":
+        raise SystemExit("bench.py --path mp2 is a single-GPU measurement (--gpus 1)")
+    ndev = torch.cuda.device_count()
+    if ndev < args.gpus and not args.share_gpu:
+        raise SystemExit(f"bench.py --gpus {args.gpus}: only {ndev} CUDA device(s) visible; one rank per GPU is "
+                         "required (no rank shares a GPU in a measurement)")
+    import socket
+    sock = socket.socket()
+    sock.bind(("127.0.0.1", 0))
+    port = sock.getsockname()[1]
+    sock.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    sys.stdout.flush()
+    os.execv(sys.executable, cmd)
 
 
 # ----------------------------------------------------------------------------- clocks
@@ -166,8 +207,9 @@ def run_reference(args, rank, world):
         times.append(dt)
     dt = float(np.mean(times))
     val = flops / dt * 1e-12
-    ntrip = (hi - lo) * (hi - lo + 1) * (hi - lo + 2) // 6
-    sample = f"one triplet {trip} of the workload per step (12 v^3 (v+o) = {flops:.3e} flops), NumPy/OpenBLAS oracle"
+    ntrip = (hi - lo) * (hi - lo + 1) * (hi - lo + 2) // 6 - (hi - lo)      # i=j=k contributes exactly 0: not counted
+    sample = (f"one triplet {trip} of the workload per step (12 v^3 (v+o) = {flops:.3e} flops; our arm's step is all "
+              f"{ntrip} of them, the TFLOP/s normalisation makes the two comparable), NumPy/OpenBLAS oracle as it stands")
     out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -250,13 +292,36 @@ def run_mp2(args):
 
 
 # ----------------------------------------------------------------------------- our arm
-# bytes per W-builder launch (4 triplets) from the one `ncu --set full` capture named in profiles/README.md:
-# 15.33 GB read + 5.25 GB written at config 5 (algorithmic: 5.27 GB of F writes + L2-shared operand reads)
-NCU_TRAFFIC_W_BUILDER = {5: 15.330726e9 + 5.248752e9}
+def ncu_traffic(config, schedule):
+    """DRAM bytes per W-builder launch from the committed `ncu --set full` capture (profiles/r2_traffic.csv:
+    config,schedule,kernel,src_sha,dram_read_bytes,dram_write_bytes,capture).  Returned only when the capture
+    was made from the sources this build was compiled from; otherwise (None, reason)."""
+    import csv
+    import hashlib
+    path = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+    if not os.path.exists(path):
+        return None, "no committed ncu capture (profiles/r2_traffic.csv absent); not measured in this run"
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_2502_17963_b200", "csrc")
+    for f in sorted(os.listdir(csrc)):
+        with open(os.path.join(csrc, f), "rb") as fh:
+            h.update(fh.read())
+    sha = h.hexdigest()[:12]
+    with open(path) as fh:
+        for row in csv.DictReader(fh):
+            if int(row["config"]) == config and row["schedule"] == schedule and row["kernel"] == "w_builder":
+                if row["src_sha"] != sha:
+                    return None, (f"profiles/r2_traffic.csv holds a capture of sources {row['src_sha']}, this build is "
+                                  f"{sha}; not measured in this run")
+                return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), (
+                    f"ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch, {row['capture']} "
+                    f"(sources {sha}); a committed capture, not measured in this run")
+    return None, f"no ncu capture of config {config} / schedule {schedule}; not measured in this run"
 
 
 def main():
     args = parse()
+    ensure_ranks(args)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -275,10 +340,21 @@ def main():
         if rank == 0:
             run_mp2(args)
         return
-    torch.cuda.set_device(local_rank)
+    gpu = 0 if args.share_gpu else local_rank
+    if gpu >= torch.cuda.device_count():
+        raise SystemExit(f"bench.py: rank {rank} needs cuda:{gpu} but only {torch.cuda.device_count()} device(s) are visible")
+    torch.cuda.set_device(gpu)
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        os.environ.setdefault("MASTER_PORT", "29531")
+        if args.backend == "nccl":
+            # NCCL's init lines (ranks, transports, NVLS) go to stderr so that stdout stays one JSON line
+            os.environ.setdefault("NCCL_DEBUG", "INFO")
+            os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+            os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
+            dist.init_process_group("nccl", device_id=torch.device("cuda", gpu))
+        else:
+            dist.init_process_group("gloo")
 
     c = CONFIGS[args.config]
     o, v, X = c["nocc"], c["nvir"], c["naux"]
@@ -289,7 +365,8 @@ def main():
     nblocks = max(1, nidx // w)
     lo = 0 if args.full else (rank % nblocks) * w
     hi = nidx if args.full else lo + w
-    if args.full and world > 1:
+    strong = args.full and world > 1        # one E(T) dealt over the ranks by whole block triples
+    if strong:
         opts = bqc.make_opts(occ_block=args.occ_block, shard_rank=rank, shard_count=world,
                              flags=sched_flags | bqc.BQC_T_FLAG_SHARD_BLOCKS)
     else:
@@ -327,7 +404,7 @@ def main():
     for _ in range(args.warmup):
         e_val = step()
     barrier()
-    sampler = ClockSampler(local_rank)
+    sampler = ClockSampler(gpu)
     sampler.start()
     launches = 0
     prof = None
@@ -379,17 +456,20 @@ def main():
         e2e_ms = (time.perf_counter() - t0) * 1e3 / args.e2e_steps
         assert e_host == e_val, "e2e result differs from the device-resident result"
 
-    # max over ranks, whole-job aggregate
-    t = torch.tensor([ms, e2e_ms or 0.0, float(flops_rank)], dtype=torch.float64, device="cuda")
+    # max over ranks, whole-job aggregate; per-rank record for the scaling / load-balance report
+    mine = {"rank": rank, "ms_per_step": ms, "e2e_ms_per_step": e2e_ms or 0.0, "flops": float(flops_rank),
+            "triplets": ntrip, "slab_blocks_formed": int(prof["form_blocks"]) if prof else 0,
+            "w_builder_ms": prof["gemm_ms"] if prof else 0.0, "launches": launches}
     if world > 1:
-        tmax = t.clone()
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone()
-        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        ms, e2e_ms_max, flops_total = float(tmax[0]), float(tmax[1]), float(tsum[2])
+        per_rank = [None] * world
+        dist.all_gather_object(per_rank, mine)
         e_total = bqc.combine_partials(e_val)              # the path's one exchange: a scalar per rank
     else:
-        e2e_ms_max, flops_total, e_total = (e2e_ms or 0.0), float(flops_rank), e_val
+        per_rank, e_total = [mine], e_val
+    ms = max(r["ms_per_step"] for r in per_rank)
+    e2e_ms_max = max(r["e2e_ms_per_step"] for r in per_rank)
+    flops_total = sum(r["flops"] for r in per_rank)
+    launches_total = sum(r["launches"] for r in per_rank)
 
     if rank == 0:
         # working set of one W-builder launch vs the 126 MB L2: slabs of the outer index + the F arrays it writes
@@ -404,12 +484,18 @@ def main():
         value = flops_total / (ms * 1e-3) * 1e-12
         flops_full = bqc.bqc_t_flops(o, v, bqc.make_opts(flags=bqc.BQC_T_FLAG_ABC_DRIVEN) if abc else None)
         gemm_tf = flops_rank / (prof["gemm_ms"] * 1e-3) * 1e-12 if prof["gemm_ms"] > 0 else None
+        traffic, traffic_src = ncu_traffic(args.config, args.schedule)
+        mean_flops = flops_total / world
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "strong" if strong else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args.config, c, lo, hi, args.full, ntrip, abc),
                        "schedule": args.schedule, "triplets_per_gpu": ntrip, "occ_block": bqc.bqc_t_plan_occ_block(o, v, X, opts),
+                       "parallelism": (f"one E(T) dealt over {world} ranks by whole block triples (BQC_T_FLAG_SHARD_BLOCKS), "
+                                       "inputs replicated, one scalar exchange" if strong else
+                                       f"{world} rank(s), one occupied window each, inputs replicated, one scalar exchange"),
                        "l2": l2_note,
                        "timing": "CUDA events on the launch stream around K bqc_t_energy_ex calls, max over ranks",
                        "pinned_host": pinned, "input_gen_s": round(gen_s, 1)},
@@ -428,17 +514,21 @@ def main():
                                         "mma.sync m8n8k4 loop on all SMs); MEASURED_PEAKS.json has no FP64 entry",
                          "launches": int(prof["gemm_launches"]),
                          "flops_per_launch": flops_rank / max(prof["gemm_launches"], 1),
-                         "traffic": None if abc else NCU_TRAFFIC_W_BUILDER.get(args.config),
-                         "traffic_source": "ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch "
-                                           "(profiles/r1c_gemm_nt_full.txt)" if (args.config in NCU_TRAFFIC_W_BUILDER
-                                                                                   and not abc)
-                                           else None},
+                         "traffic": traffic, "traffic_source": traffic_src},
             "clocks": clocks,
             "e2e": {"value": (flops_total / (e2e_ms_max * 1e-3) * 1e-12) if e2e_ms_max else None, "unit": UNIT,
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": e2e_ms_max, "steps": args.e2e_steps},
-            "gpu_launches": launches,
+            "gpu_launches": launches_total,
         }
+        if world > 1:
+            out["ranks"] = {"per_rank": per_rank,
+                            "load_imbalance_max_over_mean_flops": max(r["flops"] for r in per_rank) / mean_flops,
+                            "time_imbalance_max_over_mean": ms / (sum(r["ms_per_step"] for r in per_rank) / world),
+                            "backend": args.backend}
+            if args.share_gpu:
+                out["config"]["shared_gpu"] = ("TEST MODE: all ranks ran on cuda:0, so the timings are not a "
+                                               "multi-GPU measurement")
         if world == 1 and not args.no_cpu_baseline:
             # the oracle as it stands on three triplets of the workload (one per class i<j<k, i=j<k, i<j=k); its
             # per-triplet values are compared with the e_ijk the timed GPU steps produced (north_star tolerance)

@@ -95,13 +95,15 @@ enum {
                                    the transposed amplitude / DF arrays it needs inside the workspace
                                    (one extra copy of t2 and B_ov).                                      */
   BQC_T_FLAG_SHARD_BLOCKS = 8   /* multi-GPU sharding by whole block triples instead of single triplets: with
-                                   shard_count > 1 this call evaluates the block triples (I <= J <= K blocks
-                                   of occ_block orbitals, numbered in loop order) whose number % shard_count
-                                   == shard_rank, and forms only the (vv|ov) slabs those need — the per-triplet
-                                   modulo makes every shard form every slab.  Shards are still disjoint and
-                                   cover every triplet once; per-triplet values are the same bits.  The split
-                                   depends on occ_block (bqc_t_plan_occ_block); bqc_t_triplet_owner does not
-                                   describe it.                                                        */
+                                   shard_count > 1 the block triples (I <= J <= K blocks of occ_block orbitals)
+                                   are dealt to the ranks largest first, each to the least-loaded rank (a
+                                   deterministic function of window, occ_block and shard_count that every rank
+                                   computes identically), and a rank forms only the (vv|ov) slabs its own block
+                                   triples need — the per-triplet modulo makes every shard form every slab.
+                                   Shards are disjoint and cover every triplet once; per-triplet values are the
+                                   same bits.  With occ_block = 0 the block size is lowered from the
+                                   memory-derived one until the deal is within 3 % of even.
+                                   bqc_t_triplet_owner_ex describes the split, bqc_t_flops each rank's share. */
 };
 
 /* ---- host-only helpers (no GPU needed) -------------------------------------------------- */
@@ -112,6 +114,12 @@ BQC_API size_t bqc_t_num_triplets(int nocc);
 BQC_API size_t bqc_t_triplet_index(int nocc, int i, int j, int k);
 /* Rank that evaluates triplet (i,j,k) under `shard_count`-way sharding (-1 on bad args). */
 BQC_API int bqc_t_triplet_owner(int nocc, int shard_count, int i, int j, int k);
+/* Rank that evaluates triplet (i,j,k) under the sharding `opts` describes: the per-triplet modulo above, or,
+   with BQC_T_FLAG_SHARD_BLOCKS, the owner of its block triple (window, occ_block and shard_count taken from
+   opts; shard_rank ignored).  With BQC_T_FLAG_ABC_DRIVEN (i,j,k) is a virtual triple a<=b<=c.  -1 if the
+   triplet is outside the window or an argument is invalid.  This is the host description of the split the
+   multi-GPU path uses. */
+BQC_API int bqc_t_triplet_owner_ex(int nocc, int nvir, int naux, const bqc_t_opts* opts, int i, int j, int k);
 /* Algorithmic FP64 flop count of the W builder over the selected triplets:
    [#triplets(i<=j<=k, not i=j=k) in window/shard] * 12 v^3 (v+o). */
 BQC_API double bqc_t_flops(int nocc, int nvir, const bqc_t_opts* opts);
@@ -119,6 +127,14 @@ BQC_API double bqc_t_flops(int nocc, int nvir, const bqc_t_opts* opts);
 BQC_API int bqc_t_plan_occ_block(int nocc, int nvir, int naux, const bqc_t_opts* opts);
 /* Bytes of device workspace bqc_t_energy_ex needs for these sizes/options. */
 BQC_API size_t bqc_t_workspace_bytes(int nocc, int nvir, int naux, const bqc_t_opts* opts);
+
+/* The fixed-order sum that closes the multi-GPU path (the
+   independent pieces of (T) are split over GPUs and only their partial energies are combined):
+   *out_host = x[0] + x[1] + ... + x[n-1], added strictly left to right in FP64.  x may be a HOST or a
+   DEVICE pointer (detected; a device array is summed by a one-thread kernel on `stream`, in the same
+   order, so both give the same bits).  Used on the rank-ordered all-gather of the per-rank partial
+   energies, so that every rank returns an identical E(T).  Usable without a GPU for host arrays. */
+BQC_API int bqc_sum_in_order(const double* x, size_t n, double* out_host, void* stream);
 
 BQC_API int bqc_last_error(void);                 /* thread-local code of the last failing call (0 = none) */
 BQC_API const char* bqc_error_string(int code);   /* static description of an error code */

@@ -62,12 +62,16 @@ def lib():
     L.bqc_debug_tiling.argtypes = [c_int, POINTER(c_int), c_int]
     L.bqc_t_triplet_owner.restype = c_int
     L.bqc_t_triplet_owner.argtypes = [c_int] * 5
+    L.bqc_t_triplet_owner_ex.restype = c_int
+    L.bqc_t_triplet_owner_ex.argtypes = [c_int] * 3 + [POINTER(bqc_t_opts)] + [c_int] * 3
     L.bqc_t_flops.restype = c_double
     L.bqc_t_flops.argtypes = [c_int, c_int, POINTER(bqc_t_opts)]
     L.bqc_t_plan_occ_block.restype = c_int
     L.bqc_t_plan_occ_block.argtypes = [c_int, c_int, c_int, POINTER(bqc_t_opts)]
     L.bqc_t_workspace_bytes.restype = c_size_t
     L.bqc_t_workspace_bytes.argtypes = [c_int, c_int, c_int, POINTER(bqc_t_opts)]
+    L.bqc_sum_in_order.restype = c_int
+    L.bqc_sum_in_order.argtypes = [dp, c_size_t, POINTER(c_double), c_void_p]
     L.bqc_last_error.restype = c_int
     L.bqc_error_string.restype = c_char_p
     L.bqc_error_string.argtypes = [c_int]
@@ -179,6 +183,10 @@ def bqc_t_triplet_owner(nocc, shard_count, i, j, k):
     return lib().bqc_t_triplet_owner(nocc, shard_count, i, j, k)
 
 
+def bqc_t_triplet_owner_ex(nocc, nvir, naux, opts, i, j, k):
+    return lib().bqc_t_triplet_owner_ex(nocc, nvir, naux, _optp(opts), i, j, k)
+
+
 def bqc_t_flops(nocc, nvir, opts=None):
     return lib().bqc_t_flops(nocc, nvir, _optp(opts))
 
@@ -189,6 +197,17 @@ def bqc_t_plan_occ_block(nocc, nvir, naux, opts=None):
 
 def bqc_t_workspace_bytes(nocc, nvir, naux, opts=None):
     return lib().bqc_t_workspace_bytes(nocc, nvir, naux, _optp(opts))
+
+
+def bqc_sum_in_order(x):
+    """x[0] + x[1] + ... left to right, by the library (host loop or one-thread kernel: same bits).
+    `x`: contiguous 1-D float64 tensor, host or CUDA."""
+    if not isinstance(x, torch.Tensor) or x.dtype != torch.float64 or x.dim() != 1 or not x.is_contiguous():
+        raise ValueError("bqc_sum_in_order: need a contiguous 1-D float64 tensor")
+    out = c_double(0.0)
+    stream = _stream() if x.is_cuda else None
+    _check(lib().bqc_sum_in_order(c_void_p(x.data_ptr()), x.numel(), byref(out), stream))
+    return out.value
 
 
 def bqc_last_error():

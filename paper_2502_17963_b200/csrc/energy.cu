@@ -273,6 +273,22 @@ int launch_final_sum(const double* e_trip, long long n, double* out, cudaStream_
   return BQC_OK;
 }
 
+// ------------------------------------------------------------------ strictly sequential sum (cross-rank combine)
+// One thread adds x[0], x[1], ... left to right: the same order (and so the same bits) as the host loop of
+// bqc_sum_in_order, whatever the memory space of x.  n is a rank count, not a data size.
+__global__ void ordered_sum_kernel(const double* __restrict__ x, long long n, double* __restrict__ out) {
+  double s = 0.0;
+  for (long long i = 0; i < n; ++i) s += x[i];
+  *out = s;
+}
+
+int launch_ordered_sum(const double* x, long long n, double* out, cudaStream_t s) {
+  ordered_sum_kernel<<<1, 1, 0, s>>>(x, n, out);
+  count_launch();
+  BQC_CUDA_OK(cudaGetLastError());
+  return BQC_OK;
+}
+
 // ------------------------------------------------------------------ dense W / V of one triplet (debug)
 __global__ void assemble_wv_kernel(const double* __restrict__ F, int nb, int v, const double* __restrict__ Jjk,
                                    const double* __restrict__ Jik, const double* __restrict__ Jij,

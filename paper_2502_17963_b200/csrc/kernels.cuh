@@ -50,6 +50,9 @@ int launch_reduce_triplets(const double* partial, const TripletRec* trips, int n
 // *out = sum_n e_trip[n] in a fixed order (single block)
 int launch_final_sum(const double* e_trip, long long n, double* out, cudaStream_t s);
 
+// *out = x[0] + x[1] + ... + x[n-1], one thread, left to right (device pointers)
+int launch_ordered_sum(const double* x, long long n, double* out, cudaStream_t s);
+
 // dense W / V [v][v][v] of one triplet from its three blocked F arrays (debug / parity of rows a2, a3)
 int launch_assemble_wv(const double* F, int nbv, int v, const double* J, int nw, int pi, int pj, int pk,
                        const double* t1i, const double* t1j, const double* t1k, const double* t2, int o, int i,

@@ -103,6 +103,66 @@ int auto_occ_block(int na, int v, int Kp) {
   return ceil_div(na, nblk);   // balanced blocks
 }
 
+// Non-diagonal triplets pi <= pj <= pk of block triple (I, J, K) over na orbitals in blocks of bo.
+long long block_triple_work(int na, int bo, int I, int J, int K) {
+  auto b0 = [&](int b) { return b * bo; };
+  auto b1 = [&](int b) { return std::min(na, (b + 1) * bo); };
+  long long n = 0;
+  for (int pi = b0(I); pi < b1(I); ++pi)
+    for (int pj = std::max(pi, b0(J)); pj < b1(J); ++pj) {
+      const int k0 = std::max(pj, b0(K));
+      n += std::max(0, b1(K) - k0);
+      if (pi == pj && pj >= k0 && pj < b1(K)) --n;   // i = j = k contributes exactly 0 and is skipped
+    }
+  return n;
+}
+
+// BQC_T_FLAG_SHARD_BLOCKS: owner of every block triple I <= J <= K (numbered in loop order).  Largest block
+// triples first, each to the least-loaded rank so far (ties: lower rank) — a deterministic function of
+// (na, bo, shard_count), so every rank and the host helpers (bqc_t_flops, bqc_t_triplet_owner_ex) agree.
+std::vector<int> deal_block_triples(int na, int bo, int shard_count, std::vector<long long>* load_out = nullptr) {
+  const int nblk = ceil_div(na, bo);
+  struct BT { long long work; int id; };
+  std::vector<BT> bt;
+  int id = 0;
+  for (int I = 0; I < nblk; ++I)
+    for (int J = I; J < nblk; ++J)
+      for (int K = J; K < nblk; ++K) bt.push_back({block_triple_work(na, bo, I, J, K), id++});
+  std::vector<int> owner(bt.size(), 0);
+  std::vector<long long> load(shard_count, 0);
+  std::stable_sort(bt.begin(), bt.end(), [](const BT& a, const BT& b) { return a.work > b.work; });
+  for (const BT& t : bt) {
+    int best = 0;
+    for (int r = 1; r < shard_count; ++r)
+      if (load[r] < load[best]) best = r;
+    owner[t.id] = best;
+    load[best] += t.work;
+  }
+  if (load_out) *load_out = load;
+  return owner;
+}
+
+// Block size for a block-triple-sharded run: the largest Bo <= the memory-derived one whose deal is within
+// 3 % of even (the slabs of a block are re-formed by every rank that owns one of its triples, so larger is
+// cheaper); the best one found if none is.
+int balanced_occ_block(int na, int bo_max, int shard_count) {
+  int best_bo = bo_max;
+  double best = -1.0;
+  for (int bo = bo_max; bo >= 1; --bo) {
+    if (bo < bo_max && ceil_div(na, bo) == ceil_div(na, bo + 1)) continue;   // same block count: skip
+    std::vector<long long> load;
+    deal_block_triples(na, bo, shard_count, &load);
+    long long mx = 0, sum = 0;
+    for (long long l : load) { mx = std::max(mx, l); sum += l; }
+    if (sum == 0) return bo_max;
+    const double imb = (double)mx * shard_count / (double)sum;
+    if (best < 0 || imb < best - 1e-12) { best = imb; best_bo = bo; }
+    if (imb <= 1.03) break;
+    if (ceil_div(na, bo) > 64) break;   // enough block triples (> 45 000): stop searching
+  }
+  return best_bo;
+}
+
 int make_plan(Plan& P, int o, int v, int X, const std::vector<int>& act, const bqc_t_opts* opts) {
   P.o = o; P.v = v; P.X = X;
   P.act = act;
@@ -128,6 +188,7 @@ int make_plan(Plan& P, int o, int v, int X, const std::vector<int>& act, const b
     return BQC_ERR_INVALID_OPTION;
   }
   P.Bo = bo > 0 ? std::min(bo, P.na) : auto_occ_block(P.na, v, P.Kp);
+  if (bo == 0 && P.shard_blocks && P.shard_count > 1) P.Bo = balanced_occ_block(P.na, P.Bo, P.shard_count);
   P.nblk = ceil_div(P.na, P.Bo);
   P.nsets = P.nblk == 1 ? 1 : 4;
   P.nslots = P.nsets * P.Bo;
@@ -578,6 +639,8 @@ int Pipeline::build_schedule() {
   auto slot_of = [&](int pos, int set, int block) { return set * P.Bo + (pos - block_begin(block)); };
 
   long long block_triple = -1;
+  std::vector<int> bt_owner;
+  if (P.shard_blocks) bt_owner = deal_block_triples(na, P.Bo, P.shard_count);
   for (int I = 0; I < P.nblk; ++I) {
     for (int Jb = I; Jb < P.nblk; ++Jb) {
       const int sJ = (Jb == I) ? 0 : 1;
@@ -585,7 +648,7 @@ int Pipeline::build_schedule() {
         ++block_triple;
         // BQC_T_FLAG_SHARD_BLOCKS: whole block triples are dealt to the shards, so a shard forms only the
         // slabs of its own block triples; otherwise every shard owns some triplets of every block triple
-        if (P.shard_blocks && (int)(block_triple % P.shard_count) != P.shard_rank) continue;
+        if (P.shard_blocks && bt_owner[(size_t)block_triple] != P.shard_rank) continue;
         int sK = sJ;
         if (K != Jb) sK = (set_block[2] == K) ? 2 : (set_block[3] == K ? 3 : 2 + (kflip++ & 1));
         // triplets of this block triple owned by this shard
@@ -913,6 +976,30 @@ int bqc_t_triplet_owner(int nocc, int shard_count, int i, int j, int k) {
   return (int)(idx % (size_t)shard_count);
 }
 
+int bqc_t_triplet_owner_ex(int nocc, int nvir, int naux, const bqc_t_opts* opts, int i, int j, int k) {
+  clear_error();
+  if (check_sizes(nocc, nvir, naux) != BQC_OK) return -1;
+  if (opts && (opts->flags & BQC_T_FLAG_ABC_DRIVEN)) {   // (i,j,k) are virtual indices a<=b<=c
+    const bqc_t_opts d = dual_opts(opts);
+    return bqc_t_triplet_owner_ex(nvir, nocc, naux, &d, i, j, k);
+  }
+  int lo, hi;
+  if (resolve_window(nocc, opts, &lo, &hi) != BQC_OK) return -1;
+  if (i < lo || i > j || j > k || k >= hi) return -1;
+  const int sc = (opts && opts->shard_count > 0) ? opts->shard_count : 1;
+  if (!(opts && (opts->flags & BQC_T_FLAG_SHARD_BLOCKS)))
+    return (int)(triplet_index(nocc, i, j, k) % (size_t)sc);
+  Plan P;
+  std::vector<int> act(hi - lo);
+  for (int x = lo; x < hi; ++x) act[x - lo] = x;
+  bqc_t_opts o2 = *opts;
+  o2.shard_rank = 0;
+  if (make_plan(P, nocc, nvir, naux, act, &o2) != BQC_OK) return -1;
+  // block triples I <= J <= K are numbered in loop order = lexicographic rank among the nblk blocks
+  const size_t bt = triplet_index(P.nblk, (i - lo) / P.Bo, (j - lo) / P.Bo, (k - lo) / P.Bo);
+  return deal_block_triples(P.na, P.Bo, sc)[bt];
+}
+
 double bqc_t_flops(int nocc, int nvir, const bqc_t_opts* opts) {
   clear_error();
   if (nocc <= 0 || nvir <= 0) return 0.0;
@@ -931,18 +1018,9 @@ double bqc_t_flops(int nocc, int nvir, const bqc_t_opts* opts) {
     std::vector<int> act(hi - lo);
     for (int x = lo; x < hi; ++x) act[x - lo] = x;
     if (make_plan(P, nocc, nvir, 1, act, opts) != BQC_OK) return -1.0;
-    auto b0 = [&](int b) { return b * P.Bo; };
-    auto b1 = [&](int b) { return std::min(P.na, (b + 1) * P.Bo); };
-    long long bt = -1;
-    for (int I = 0; I < P.nblk; ++I)
-      for (int J = I; J < P.nblk; ++J)
-        for (int K = J; K < P.nblk; ++K) {
-          if ((int)(++bt % sc) != sr) continue;
-          for (int pi = b0(I); pi < b1(I); ++pi)
-            for (int pj = std::max(pi, b0(J)); pj < b1(J); ++pj)
-              for (int pk = std::max(pj, b0(K)); pk < b1(K); ++pk)
-                if (!(pi == pj && pj == pk)) ++n;
-        }
+    std::vector<long long> load;
+    deal_block_triples(P.na, P.Bo, sc, &load);
+    n = (size_t)load[sr];
     const double v = nvir;
     return (double)n * 12.0 * v * v * v * (v + nocc);
   }
@@ -987,6 +1065,41 @@ size_t bqc_t_workspace_bytes(int nocc, int nvir, int naux, const bqc_t_opts* opt
   for (int x = lo; x < hi; ++x) act[x - lo] = x;
   if (make_plan(P, nocc, nvir, naux, act, opts) != BQC_OK) return 0;
   return P.total;
+}
+
+int bqc_sum_in_order(const double* x, size_t n, double* out_host, void* stream_v) {
+  clear_error();
+  if (!out_host || (!x && n > 0)) {
+    set_error(BQC_ERR_NULL_POINTER, "bqc_sum_in_order: %s is NULL", out_host ? "x" : "out_host");
+    return BQC_ERR_NULL_POINTER;
+  }
+  if (n == 0) {
+    *out_host = 0.0;
+    return BQC_OK;
+  }
+  cudaPointerAttributes attr;
+  const cudaError_t e = cudaPointerGetAttributes(&attr, x);
+  if (e != cudaSuccess) cudaGetLastError();   // no driver / no device: x can only be host memory
+  if (e == cudaSuccess && (attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged)) {
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
+    double* d = nullptr;
+    BQC_CUDA_OK(cudaMallocAsync(&d, 8, stream));
+    int rc = launch_ordered_sum(x, (long long)n, d, stream);
+    if (rc == BQC_OK) {
+      cudaError_t c = cudaMemcpyAsync(out_host, d, 8, cudaMemcpyDeviceToHost, stream);
+      if (c == cudaSuccess) c = cudaStreamSynchronize(stream);
+      if (c != cudaSuccess) {
+        set_error(BQC_ERR_CUDA, "bqc_sum_in_order: %s", cudaGetErrorString(c));
+        rc = BQC_ERR_CUDA;
+      }
+    }
+    cudaFreeAsync(d, stream);
+    return rc;
+  }
+  double s = 0.0;
+  for (size_t i = 0; i < n; ++i) s += x[i];   // the same left-to-right order as ordered_sum_kernel
+  *out_host = s;
+  return BQC_OK;
 }
 
 int bqc_t_last_profile(double* out, int n) {

@@ -4,8 +4,8 @@ Triplets are independent, so each rank evaluates its share of them (`bqc_t_opts.
 shard_count`; by default whole block triples, `BQC_T_FLAG_SHARD_BLOCKS`, so that a rank forms only the
 (vv|ov) slabs its own triplets need) on its own replica of the inputs and there is no data-path
 collective.  The only exchange is the final scalar: the per-rank partial sums are all-gathered and
-added in rank order, so every rank returns the same bits and the result does not depend on arrival
-order (an 8-byte all-reduce would do when that is not required).  Argument marshalling and
+added in rank order by the library (`bqc_sum_in_order`), so every rank returns the same bits and the
+result does not depend on arrival order (an 8-byte all-reduce would do when that is not required).  Argument marshalling and
 `torch.distributed` plumbing only — every step of the (T) path runs in the CUDA library.
 """
 from __future__ import annotations
@@ -24,12 +24,9 @@ def combine_partials(e_local: float, group=None, device=None) -> float:
     if device is None:
         device = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend(group) == "nccl" else "cpu"
     mine = torch.tensor([e_local], dtype=torch.float64, device=device)
-    parts = [torch.zeros_like(mine) for _ in range(world)]
-    dist.all_gather(parts, mine, group=group)
-    total = 0.0
-    for p in parts:            # fixed order: rank 0, 1, ...
-        total += float(p.item())
-    return total
+    parts = torch.zeros(world, dtype=torch.float64, device=device)
+    dist.all_gather_into_tensor(parts, mine, group=group)
+    return _b.bqc_sum_in_order(parts)      # the library's fixed-order sum: rank 0, 1, ... left to right
 
 
 def bqc_t_energy_sharded(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, group=None,
