@@ -60,8 +60,9 @@ enum {
 
 /* Options of bqc_t_energy_ex.  Zero-initialise for defaults. */
 typedef struct bqc_t_opts {
-  int occ_block;     /* occupied block size Bo of the slab cache (0 = auto).  4*Bo (vv|ov)
-                        slabs are resident at a time; the full O(o v^3) tensor never is.     */
+  int occ_block;     /* occupied block size Bo of the slab cache (0 = auto from workspace_gib).  4*Bo
+                        (vv|ov) slabs and the B~ / (ov|ov) blocks of 16 Bo^2 orbital pairs are resident
+                        at a time; the full O(o v^3) and O(o^2 v^2) tensors never are.          */
   int occ_lo;        /* restrict to triplets with occ_lo <= i <= j <= k < occ_hi;            */
   int occ_hi;        /*   occ_lo = occ_hi = 0 means all occupied orbitals.                   */
   int shard_rank;    /* multi-GPU sharding: this call evaluates the triplets whose index     */
@@ -69,7 +70,9 @@ typedef struct bqc_t_opts {
                         (BQC_T_FLAG_SHARD_BLOCKS deals whole block triples instead.)         */
   int max_batch;     /* triplets per W-builder launch (0 = auto from memory)                 */
   int flags;         /* BQC_T_FLAG_* below                                                   */
-  int reserved;
+  int workspace_gib; /* soft cap, in GiB, on the buffers whose size follows occ_block (slab cache + pair
+                        blocks) when occ_block = 0; 0 = 36.  The fixed part (K-major DF copies, one batch
+                        of F arrays) comes on top: bqc_t_workspace_bytes reports the total.          */
   const double* f_ov;/* non-canonical reference (Eqs. (5),(7); reading G15): the
                         occupied-virtual Fock block f[i,a], [nocc][nvir], caller-owned, read-only;
                         DEVICE memory for bqc_t_energy_ex, HOST memory for bqc_t_energy_host.
@@ -85,15 +88,16 @@ enum {
                                    §8(f) NEXT-2): the outer loop runs over virtual triples a<=b<=c with all
                                    o^3 occupied triples inside, instead of occupied triplets i<=j<=k with
                                    all v^3 virtual triples inside.  Same E(T) up to summation order; the
-                                   resident pieces are o^2 (v+o) per virtual instead of v^2 (v+o) per
-                                   occupied orbital, which is what large virtual spaces (cc-pVTZ/QZ-shaped
-                                   inputs) need.  With this flag occ_block / occ_lo / occ_hi / shard_* refer
-                                   to the VIRTUAL index, e_triplet_dev has bqc_t_num_triplets(nvir) entries
-                                   indexed by bqc_t_triplet_index(nvir, a, b, c) and holds the weighted
+                                   resident pieces are o^2 (v+o) per virtual orbital of a block instead of
+                                   v^2 (v+o) per occupied orbital, and O(Bv^2 o (v+o)) for the pairs of the
+                                   4 resident virtual blocks of Bv orbitals — nothing of size o v^3 or
+                                   v^2 o^2 is stored, no transposed copy of t2 or B_vv is made — which is
+                                   what large virtual spaces (cc-pVTZ/QZ-shaped inputs) need.  With this flag
+                                   occ_block / occ_lo / occ_hi / shard_* refer to the VIRTUAL index,
+                                   e_triplet_dev has bqc_t_num_triplets(nvir) entries indexed by
+                                   bqc_t_triplet_index(nvir, a, b, c) and holds the weighted
                                    per-virtual-triple contributions (2 - d_ab - d_bc) sum_ijk R V / D, and
-                                   bqc_t_flops counts 12 o^3 (v+o) per virtual triple.  The library builds
-                                   the transposed amplitude / DF arrays it needs inside the workspace
-                                   (one extra copy of t2 and B_ov).                                      */
+                                   bqc_t_flops counts 12 o^3 (v+o) per virtual triple.                   */
   BQC_T_FLAG_SHARD_BLOCKS = 8   /* multi-GPU sharding by whole block triples instead of single triplets: with
                                    shard_count > 1 the block triples (I <= J <= K blocks of occ_block orbitals)
                                    are dealt to the ranks largest first, each to the least-loaded rank (a
@@ -147,7 +151,8 @@ BQC_API const char* bqc_version(void);
      eps_occ [nocc], eps_vir [nvir], t1 [nocc][nvir], t2 [nocc][nocc][nvir][nvir],
      B_oo [naux][nocc][nocc], B_ov [naux][nocc][nvir]  (B_ov[Q,i,a] = B[Q,i,nocc+a]),
      B_vv [naux][nvir][nvir].
-   Workspace is allocated on the device internally and freed before return.
+   Workspace is allocated on the device internally; it is freed before return when larger than 2 GiB and
+   otherwise kept with the thread's cached plan for the next call (bqc_release_cached frees it).
    nocc == 1 is valid and returns exactly 0.0 (no triples with two electrons). */
 BQC_API double bqc_t_energy(int nocc, int nvir, int naux,
                     const double* eps_occ, const double* eps_vir,
@@ -170,12 +175,32 @@ BQC_API int bqc_t_energy_ex(int nocc, int nvir, int naux,
                     const bqc_t_opts* opts, void* workspace, size_t workspace_bytes,
                     double* e_total_host, double* e_triplet_dev, void* stream);
 
+/* Reusable plan (PAPER.md:177 on the cost of allocations inside a loop): everything of an
+   evaluation that does not depend on the VALUES of the inputs — workspace (caller's, or allocated once here
+   when workspace == NULL), helper stream, events, tensor maps, the block-triple schedule — is built once by
+   bqc_t_plan_create and reused by every bqc_t_plan_execute on the same device.  Array arguments and results
+   are as for bqc_t_energy_ex; f_ov must be non-NULL exactly when the plan was created with opts->f_ov set
+   (only its NULL-ness is recorded at creation).  A plan is used by one thread at a time.
+   bqc_t_energy_ex keeps the plan of the thread's last call and reuses it when sizes, options, workspace and
+   device repeat (a plan that owns more than 2 GiB of workspace is dropped when its call returns);
+   bqc_release_cached() frees it. */
+typedef struct bqc_t_plan_s* bqc_t_plan;
+BQC_API int bqc_t_plan_create(int nocc, int nvir, int naux, const bqc_t_opts* opts,
+                      void* workspace, size_t workspace_bytes, bqc_t_plan* plan_out);
+BQC_API int bqc_t_plan_execute(bqc_t_plan plan,
+                      const double* eps_occ, const double* eps_vir, const double* t1, const double* t2,
+                      const double* B_oo, const double* B_ov, const double* B_vv, const double* f_ov,
+                      double* e_total_host, double* e_triplet_dev, void* stream);
+BQC_API void bqc_t_plan_destroy(bqc_t_plan plan);
+BQC_API size_t bqc_t_plan_workspace_bytes(bqc_t_plan plan);   /* bytes of device workspace the plan uses */
+BQC_API void bqc_release_cached(void);                         /* drop this thread's cached plan */
+
 /* Timing of the last bqc_t_energy_ex call of this thread that had BQC_T_FLAG_PROFILE set, measured
    with CUDA events on the streams the kernels were launched on.  Fills up to n (<= 9) doubles:
      [0] W-builder (tile-GEMM) kernel milliseconds, summed over launches   [1] number of those launches
      [2] energy-contraction + per-triplet reduction kernel milliseconds     [3] number of those launches
-     [4] slab-former milliseconds (DF GEMM + hole columns, former stream)   [5] number of slab blocks formed
-     [6] input repacking + B~/J formation milliseconds                      [7] whole call, first to last kernel
+     [4] slab-former + B~/J pair-block former milliseconds (DF GEMMs)       [5] number of slab blocks formed
+     [6] input repacking milliseconds                                       [7] whole call, first to last kernel
      [8] number of library kernels launched by the call (counted whether or not PROFILE was set)
    Returns the number of values written (n <= 9). */
 BQC_API int bqc_t_last_profile(double* out, int n);

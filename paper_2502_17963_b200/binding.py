@@ -26,7 +26,7 @@ class BqcError(RuntimeError):
 class bqc_t_opts(Structure):
     _fields_ = [("occ_block", c_int), ("occ_lo", c_int), ("occ_hi", c_int),
                 ("shard_rank", c_int), ("shard_count", c_int), ("max_batch", c_int),
-                ("flags", c_int), ("reserved", c_int), ("f_ov", c_void_p)]
+                ("flags", c_int), ("workspace_gib", c_int), ("f_ov", c_void_p)]
 
 
 class bqc_mp2_opts(Structure):
@@ -147,10 +147,11 @@ def _inputs(nocc, nvir, naux, arrays, device):
     return [_ptr(t, s, n, device) for t, s, n in zip(arrays, _shapes(nocc, nvir, naux), _NAMES)]
 
 
-def make_opts(occ_block=0, occ_lo=0, occ_hi=0, shard_rank=0, shard_count=1, max_batch=0, flags=0, f_ov=None):
+def make_opts(occ_block=0, occ_lo=0, occ_hi=0, shard_rank=0, shard_count=1, max_batch=0, flags=0, f_ov=None,
+              workspace_gib=0):
     """`f_ov`: optional [nocc, nvir] float64 tensor (CUDA for bqc_t_energy_ex, host for bqc_t_energy_host);
     the returned struct keeps a reference so the pointer stays valid."""
-    o = bqc_t_opts(occ_block, occ_lo, occ_hi, shard_rank, shard_count, max_batch, flags, 0, None)
+    o = bqc_t_opts(occ_block, occ_lo, occ_hi, shard_rank, shard_count, max_batch, flags, workspace_gib, None)
     if f_ov is not None:
         if f_ov.dtype != torch.float64 or not f_ov.is_contiguous() or f_ov.dim() != 2:
             raise ValueError("f_ov must be a contiguous float64 [nocc, nvir] tensor")

@@ -130,8 +130,11 @@ __global__ void __launch_bounds__(kEThreads, kFock ? 3 : 4) energy_kernel(const 
         // T^(0) = t2[j,k], T^(1) = t2[i,k], T^(2) = t2[i,j]
         const int ox = (m == 0) ? tr.j : tr.i;
         const int oy = (m == 2) ? tr.j : tr.k;
-        const double* Tm = a.t2 + ((size_t)ox * a.o + oy) * v * v;
-        fk.Tt[m][pr][lu * kJPitch + lw] = (gu < v && gw < v) ? __ldg(Tm + (size_t)gu * v + gw) : 0.0;
+        double tval = 0.0;
+        if (gu < v && gw < v)
+          tval = a.dual ? -__ldg(a.t2 + (((size_t)gu * v + gw) * a.o + ox) * a.o + oy)   // -t2c[u,w,x,y]
+                        : __ldg(a.t2 + (((size_t)ox * a.o + oy) * v + gu) * v + gw);
+        fk.Tt[m][pr][lu * kJPitch + lw] = tval;
       }
     }
   }
@@ -268,6 +271,43 @@ __global__ void final_sum_kernel(const double* __restrict__ e, long long n, doub
 
 int launch_final_sum(const double* e_trip, long long n, double* out, cudaStream_t s) {
   final_sum_kernel<<<1, 1024, 0, s>>>(e_trip, n, out);
+  count_launch();
+  BQC_CUDA_OK(cudaGetLastError());
+  return BQC_OK;
+}
+
+// ------------------------------------------------------------------ denominator bound on the stream (reading G10)
+// out[0] = 1 if 3 max(eps_occ) - 3 min(eps_vir) >= 0 (or not comparable: NaN), else 0; out[1] = max eps_occ,
+// out[2] = min eps_vir.  One block; max/min are order-independent, so the result is deterministic.
+__global__ void denominator_check_kernel(const double* __restrict__ eps_occ, int o, const double* __restrict__ eps_vir,
+                                         int v, double* __restrict__ out) {
+  __shared__ double smax[256], smin[256];
+  __shared__ int snan[256];
+  double mx = -INFINITY, mn = INFINITY;
+  int bad = 0;
+  for (int i = threadIdx.x; i < o; i += 256) { const double e = eps_occ[i]; bad |= (e != e); mx = fmax(mx, e); }
+  for (int a = threadIdx.x; a < v; a += 256) { const double e = eps_vir[a]; bad |= (e != e); mn = fmin(mn, e); }
+  smax[threadIdx.x] = mx; smin[threadIdx.x] = mn; snan[threadIdx.x] = bad;
+  __syncthreads();
+  for (int off = 128; off > 0; off >>= 1) {
+    if (threadIdx.x < off) {
+      smax[threadIdx.x] = fmax(smax[threadIdx.x], smax[threadIdx.x + off]);
+      smin[threadIdx.x] = fmin(smin[threadIdx.x], smin[threadIdx.x + off]);
+      snan[threadIdx.x] |= snan[threadIdx.x + off];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    const bool ok = !snan[0] && (3.0 * smax[0] - 3.0 * smin[0] < 0.0);
+    out[0] = ok ? 0.0 : 1.0;
+    out[1] = smax[0];
+    out[2] = smin[0];
+  }
+}
+
+int launch_denominator_check(const double* eps_occ, int o, const double* eps_vir, int v, double* out,
+                             cudaStream_t s) {
+  denominator_check_kernel<<<1, 256, 0, s>>>(eps_occ, o, eps_vir, v, out);
   count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;

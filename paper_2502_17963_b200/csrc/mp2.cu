@@ -260,7 +260,7 @@ static int mp2_impl(int o, int v, int X, const double* eps_occ, const double* ep
   }
   BQC_CUDA_OK(cudaMemsetAsync(e_pair, 0, (size_t)o * o * 8, s));
   BQC_CUDA_OK(cudaMemsetAsync(e_w, 0, (size_t)o * o * 8, s));
-  BQC_TRY(launch_transpose_pad(B_ov, bt, X, o * v, Xp, s));   // Bt_ov[(i,a)][Q], zero-padded to Xp
+  BQC_TRY(launch_transpose_pad(B_ov, (long long)o * v, 0, (long long)o * v, bt, X, Xp, 0, 0, s));   // Bt_ov[(i,a)][Q], zero-padded to Xp
   ++nlaunch;
 
   int ngemm = 0;

@@ -4,25 +4,41 @@
 
 namespace bqc {
 
-// ---------------------------------------------------------------- [nq][nr] -> [nr][qp] (zero pad)
-__global__ void transpose_pad_kernel(const double* __restrict__ in, double* __restrict__ out, int nq,
-                                     int nr, int qp) {
+// ---------------------------------------------------------------- [nq][in_pitch] -> [nr][qp] (zero pad)
+// out[row(r)][q] = in[q][r0 + r], r < nr, q < nq; zero for nq <= q < qp.  row(r) = r, or, with perm_v > 0, the
+// pair-transposed row: r0 + r = i * perm_v + a  ->  row = a * perm_o + i  (B_ov[Q,i,a] -> Bt_ov'[(a,i)][Q], the
+// particle-hole dual used by the abc-driven schedule).
+__global__ void transpose_pad_kernel(const double* __restrict__ in, long long in_pitch, long long r0,
+                                     double* __restrict__ out, int nq, long long nr, int qp, int perm_v,
+                                     int perm_o) {
   __shared__ double tile[32][33];
-  const int r0 = blockIdx.x * 32, q0 = blockIdx.y * 32;
+  const long long rb = (long long)blockIdx.x * 32;
+  const int q0 = blockIdx.y * 32;
   for (int dy = threadIdx.y; dy < 32; dy += blockDim.y) {
-    const int q = q0 + dy, r = r0 + threadIdx.x;
-    tile[dy][threadIdx.x] = (q < nq && r < nr) ? in[(size_t)q * nr + r] : 0.0;
+    const int q = q0 + dy;
+    const long long r = rb + threadIdx.x;
+    tile[dy][threadIdx.x] = (q < nq && r < nr) ? in[(size_t)q * in_pitch + r0 + r] : 0.0;
   }
   __syncthreads();
   for (int dy = threadIdx.y; dy < 32; dy += blockDim.y) {
-    const int r = r0 + dy, q = q0 + threadIdx.x;
-    if (r < nr && q < qp) out[(size_t)r * qp + q] = tile[threadIdx.x][dy];
+    const long long r = rb + dy;
+    const int q = q0 + threadIdx.x;
+    if (r < nr && q < qp) {
+      long long row = r;
+      if (perm_v > 0) {
+        const long long c = r0 + r;
+        row = (c % perm_v) * perm_o + c / perm_v;
+      }
+      out[(size_t)row * qp + q] = tile[threadIdx.x][dy];
+    }
   }
 }
 
-int launch_transpose_pad(const double* in, double* out, int nq, int nr, int qp, cudaStream_t s) {
-  dim3 grid(ceil_div(nr, 32), ceil_div(qp, 32));
-  transpose_pad_kernel<<<grid, dim3(32, 8), 0, s>>>(in, out, nq, nr, qp);
+int launch_transpose_pad(const double* in, long long in_pitch, long long r0, long long nr, double* out, int nq,
+                         int qp, int perm_v, int perm_o, cudaStream_t s) {
+  if (nr <= 0) return BQC_OK;
+  dim3 grid((unsigned)((nr + 31) / 32), ceil_div(qp, 32));
+  transpose_pad_kernel<<<grid, dim3(32, 8), 0, s>>>(in, in_pitch, r0, out, nq, nr, qp, perm_v, perm_o);
   count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
@@ -62,23 +78,56 @@ int launch_transpose_scale(const double* in, double* out, int batch, long long n
   return BQC_OK;
 }
 
-// ---------------------------------------------------------------- t2 rows -> Btilde rows
-__global__ void btilde_t2_kernel(const double* __restrict__ t2, double* __restrict__ btil, int o, int v,
-                                 const int* __restrict__ act, int na, int kp) {
-  // one block per (pair, r) row
+// ---------------------------------------------------------------- t2 rows -> particle columns of B~
+// B~[(sz0 + z) * nslots + (sy0 + y)][r][d] = t2[z0 + z][y0 + y][r][d],  d < v  (row pitch kp; columns >= v untouched)
+__global__ void btilde_t2_kernel(const double* __restrict__ t2, double* __restrict__ btil, int o, int v, int kp,
+                                 int nslots, int z0, int y0, int ny, int sz0, int sy0) {
+  // one block per (z, y, r) row
   const long long row = blockIdx.x;
   const int r = (int)(row % v);
-  const int pair = (int)(row / v);
-  const int z = act[pair / na], y = act[pair % na];
-  const double* src = t2 + (((size_t)z * o + y) * v + r) * v;
-  double* dst = btil + (size_t)row * kp;
+  const int zy = (int)(row / v);
+  const int z = zy / ny, y = zy % ny;
+  const double* src = t2 + (((size_t)(z0 + z) * o + (y0 + y)) * v + r) * v;
+  double* dst = btil + (((size_t)(sz0 + z) * nslots + (sy0 + y)) * v + r) * kp;
   for (int d = threadIdx.x; d < v; d += blockDim.x) dst[d] = src[d];
 }
 
-int launch_btilde_t2(const double* t2, double* btil, int o, int v, const int* act_dev, int na, int kp,
-                     cudaStream_t s) {
-  const long long rows = (long long)na * na * v;
-  btilde_t2_kernel<<<(unsigned)rows, 128, 0, s>>>(t2, btil, o, v, act_dev, na, kp);
+// abc-driven schedule (pipeline o = nvir, v = nocc; t2c = the caller's t2[nocc][nocc][nvir][nvir]):
+// B~[(sz0+z) * nslots + (sy0+y)][r][d] = t2'[z0+z][y0+y][r][d] = -t2c[r][d][z0+z][y0+y]
+// A 32 x 32 tile over (d, y) through shared memory: reads run along y, writes along d.
+__global__ void btilde_t2_dual_kernel(const double* __restrict__ t2c, double* __restrict__ btil, int o, int v,
+                                      int kp, int nslots, int z0, int y0, int ny, int sz0, int sy0) {
+  __shared__ double tile[32][33];
+  const int z = blockIdx.z / v, r = blockIdx.z % v;
+  const int yb = blockIdx.x * 32, db = blockIdx.y * 32;
+  const size_t o2 = (size_t)o * o;
+  for (int dy = threadIdx.y; dy < 32; dy += blockDim.y) {
+    const int d = db + dy, y = yb + threadIdx.x;
+    tile[dy][threadIdx.x] =
+        (d < v && y < ny) ? t2c[((size_t)r * v + d) * o2 + (size_t)(z0 + z) * o + (y0 + y)] : 0.0;
+  }
+  __syncthreads();
+  for (int dy = threadIdx.y; dy < 32; dy += blockDim.y) {
+    const int y = yb + dy, d = db + threadIdx.x;
+    if (y < ny && d < v)
+      btil[(((size_t)(sz0 + z) * nslots + (sy0 + y)) * v + r) * kp + d] = -tile[threadIdx.x][dy];
+  }
+}
+
+int launch_btilde_t2(const double* t2, double* btil, int o, int v, int kp, int nslots, int z0, int nz, int y0,
+                     int ny, int sz0, int sy0, bool dual, cudaStream_t s) {
+  if (nz <= 0 || ny <= 0) return BQC_OK;
+  if (!dual) {
+    const long long rows = (long long)nz * ny * v;
+    btilde_t2_kernel<<<(unsigned)rows, 128, 0, s>>>(t2, btil, o, v, kp, nslots, z0, y0, ny, sz0, sy0);
+  } else {
+    if ((long long)nz * v > 65535) {
+      set_error(BQC_ERR_INVALID_SIZE, "B~ block of %d x %d rows exceeds the launch grid", nz, v);
+      return BQC_ERR_INVALID_SIZE;
+    }
+    dim3 grid(ceil_div(ny, 32), ceil_div(v, 32), nz * v);
+    btilde_t2_dual_kernel<<<grid, dim3(32, 8), 0, s>>>(t2, btil, o, v, kp, nslots, z0, y0, ny, sz0, sy0);
+  }
   count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
@@ -108,12 +157,28 @@ __global__ void slab_holes_kernel(const double* __restrict__ t2, double* __restr
   }
 }
 
-int launch_slab_holes(const double* t2, double* slabs, int o, int v, int kp, int x0, int nx,
-                      int slot0, cudaStream_t s) {
+// abc-driven schedule: slab[slot][(p,q)][v + l] = -t2'[x][l][p][q] = +t2c[p][q][x][l]: a row copy
+// (pipeline o = nvir rows of length o, one per (slot, p, q)).
+__global__ void slab_holes_dual_kernel(const double* __restrict__ t2c, double* __restrict__ slabs, int o, int v,
+                                       int kp, int x0, int slot0) {
+  const size_t pq = blockIdx.x;
+  const int s = blockIdx.y;
+  const double* src = t2c + (pq * o + (size_t)(x0 + s)) * o;
+  double* dst = slabs + ((size_t)(slot0 + s) * v * v + pq) * kp + v;
+  for (int l = threadIdx.x; l < o; l += blockDim.x) dst[l] = src[l];
+}
+
+int launch_slab_holes(const double* t2, double* slabs, int o, int v, int kp, int x0, int nx, int slot0, bool dual,
+                      cudaStream_t s) {
   if (nx <= 0) return BQC_OK;
   const size_t v2 = (size_t)v * v;
-  dim3 grid((unsigned)((v2 + 31) / 32), ceil_div(o, 32), nx);
-  slab_holes_kernel<<<grid, dim3(32, 8), 0, s>>>(t2, slabs, o, v, kp, x0, slot0);
+  if (!dual) {
+    dim3 grid((unsigned)((v2 + 31) / 32), ceil_div(o, 32), nx);
+    slab_holes_kernel<<<grid, dim3(32, 8), 0, s>>>(t2, slabs, o, v, kp, x0, slot0);
+  } else {
+    dim3 grid((unsigned)v2, nx);
+    slab_holes_dual_kernel<<<grid, 128, 0, s>>>(t2, slabs, o, v, kp, x0, slot0);
+  }
   count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;

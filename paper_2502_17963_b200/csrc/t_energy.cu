@@ -1,4 +1,4 @@
-// t_energy.cu — planner, triplet-block scheduler and C ABI of libbqc_t.so.
+// t_energy.cu — the triplet-block scheduler ("engine") and the C ABI of the (T) energy.
 //
 // How W is built:
 //   augmented slab   I~_x[p,q,kappa] : kappa <  v      -> (x p|q d)                 (DF slab former, a1)
@@ -8,16 +8,25 @@
 //   F(x,y,z)[p,q,r] = sum_kappa I~_x[p,q,kappa] B~_zy[r,kappa] + sum_kappa I~_y[q,p,kappa] B~_zx[r,kappa]
 //   W_ijk[a,b,c]    = F(i,j,k)[a,b,c] + F(i,k,j)[a,c,b] + F(j,k,i)[b,c,a]          (= PAPER.md Eq. (2), G1/G5)
 // i.e. the six particle and six hole contractions of Eq. (2) become six K = v+o tile-GEMM terms.
+//
+// What is resident: the outer orbitals are cut into blocks of Bo; block triples I <= J <= K are
+// walked in order with a cache of 4 slab sets (I -> set 0, J -> set 1, K alternating 2/3) formed on a second
+// stream, and the B~ / J pair blocks of the set pairs a block triple touches, formed on the main stream just
+// before their first use.  Nothing scales with (outer extent)^2: the full (vv|ov), (ov|ov) and B~ tensors are
+// never stored.  The abc-driven schedule is the same engine on the particle-hole dual problem
+// (Plan::dual), reading the caller's arrays through dual-aware packing kernels — no transposed copy of t2.
 #include <limits.h>
 #include <math.h>
 #include <stdarg.h>
 #include <string.h>
 
 #include <algorithm>
+#include <memory>
 #include <vector>
 
 #include "gemm_nt.cuh"
 #include "kernels.cuh"
+#include "plan.cuh"
 
 namespace bqc {
 
@@ -40,195 +49,6 @@ void clear_error() {
 static thread_local double g_profile[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
 static thread_local long long g_launches = 0;
 void count_launch(int n) { g_launches += n; }
-
-namespace {
-
-// ------------------------------------------------------------------ plan
-struct Plan {
-  int o = 0, v = 0, X = 0;
-  std::vector<int> act;        // active occupied orbitals (sorted); triplets are drawn from these
-  int na = 0;                  // act.size()
-  int Xp = 0, Kp = 0;          // aux / (v+o) extents padded to multiples of 16
-  int nbv = 0;                 // 8-blocks per virtual dimension
-  size_t fsz = 0;              // doubles per blocked F array
-  size_t slab_elems = 0;       // v*v*Kp
-  int Bo = 0, nblk = 0, nsets = 0, nslots = 0;
-  int nbatch = 0;              // triplets per W-builder launch
-  int norbits = 0;
-  int use_t1 = 1;
-  int profile = 0;
-  int shard_rank = 0, shard_count = 1;
-  int shard_blocks = 0;        // BQC_T_FLAG_SHARD_BLOCKS
-  // workspace offsets (bytes)
-  size_t off_btvv = 0, off_btov = 0, off_btoo = 0, off_btil = 0, off_J = 0, off_slabs = 0, off_F = 0,
-         off_partial = 0, off_etrip = 0, off_esum = 0, off_act = 0, off_orbits = 0, off_tasks = 0,
-         off_trips = 0, total = 0;
-  size_t max_tasks = 0, max_trips = 0;
-};
-
-size_t num_triplets(int o) { return (size_t)o * (o + 1) * (o + 2) / 6; }
-
-size_t triplet_index(int o, int i, int j, int k) {
-  // lexicographic rank of (i,j,k), i<=j<=k<o
-  auto below = [&](int m) { return (size_t)m * (m + 1) * (m + 2) / 6; };   // #triplets over m orbitals
-  // triplets whose first index < i: all triplets over o minus those over (o - i) shifted
-  size_t r = below(o) - below(o - i);
-  // first index == i, second index in [i, j): for second index s the third runs over (o - s) values
-  const size_t n1 = (size_t)(o - i), n2 = (size_t)(o - j);
-  r += n1 * (n1 + 1) / 2 - n2 * (n2 + 1) / 2;
-  r += (size_t)(k - j);
-  return r;
-}
-
-int resolve_window(int o, const bqc_t_opts* opts, int* lo, int* hi) {
-  *lo = 0;
-  *hi = o;
-  if (opts && !(opts->occ_lo == 0 && opts->occ_hi == 0)) {
-    *lo = opts->occ_lo;
-    *hi = opts->occ_hi;
-  }
-  if (*lo < 0 || *hi > o || *lo >= *hi) {
-    set_error(BQC_ERR_INVALID_OPTION, "occupied window [%d,%d) invalid for nocc=%d", *lo, *hi, o);
-    return BQC_ERR_INVALID_OPTION;
-  }
-  return BQC_OK;
-}
-
-int auto_occ_block(int na, int v, int Kp) {
-  // 4*Bo augmented slabs resident; keep them under ~24 GiB
-  const double slab_bytes = (double)v * v * Kp * 8.0;
-  int bo = (int)floor(24.0 * 1073741824.0 / (4.0 * slab_bytes));
-  bo = std::max(1, std::min(bo, na));
-  const int nblk = ceil_div(na, bo);
-  return ceil_div(na, nblk);   // balanced blocks
-}
-
-// Non-diagonal triplets pi <= pj <= pk of block triple (I, J, K) over na orbitals in blocks of bo.
-long long block_triple_work(int na, int bo, int I, int J, int K) {
-  auto b0 = [&](int b) { return b * bo; };
-  auto b1 = [&](int b) { return std::min(na, (b + 1) * bo); };
-  long long n = 0;
-  for (int pi = b0(I); pi < b1(I); ++pi)
-    for (int pj = std::max(pi, b0(J)); pj < b1(J); ++pj) {
-      const int k0 = std::max(pj, b0(K));
-      n += std::max(0, b1(K) - k0);
-      if (pi == pj && pj >= k0 && pj < b1(K)) --n;   // i = j = k contributes exactly 0 and is skipped
-    }
-  return n;
-}
-
-// BQC_T_FLAG_SHARD_BLOCKS: owner of every block triple I <= J <= K (numbered in loop order).  Largest block
-// triples first, each to the least-loaded rank so far (ties: lower rank) — a deterministic function of
-// (na, bo, shard_count), so every rank and the host helpers (bqc_t_flops, bqc_t_triplet_owner_ex) agree.
-std::vector<int> deal_block_triples(int na, int bo, int shard_count, std::vector<long long>* load_out = nullptr) {
-  const int nblk = ceil_div(na, bo);
-  struct BT { long long work; int id; };
-  std::vector<BT> bt;
-  int id = 0;
-  for (int I = 0; I < nblk; ++I)
-    for (int J = I; J < nblk; ++J)
-      for (int K = J; K < nblk; ++K) bt.push_back({block_triple_work(na, bo, I, J, K), id++});
-  std::vector<int> owner(bt.size(), 0);
-  std::vector<long long> load(shard_count, 0);
-  std::stable_sort(bt.begin(), bt.end(), [](const BT& a, const BT& b) { return a.work > b.work; });
-  for (const BT& t : bt) {
-    int best = 0;
-    for (int r = 1; r < shard_count; ++r)
-      if (load[r] < load[best]) best = r;
-    owner[t.id] = best;
-    load[best] += t.work;
-  }
-  if (load_out) *load_out = load;
-  return owner;
-}
-
-// Block size for a block-triple-sharded run: the largest Bo <= the memory-derived one whose deal is within
-// 3 % of even (the slabs of a block are re-formed by every rank that owns one of its triples, so larger is
-// cheaper); the best one found if none is.
-int balanced_occ_block(int na, int bo_max, int shard_count) {
-  int best_bo = bo_max;
-  double best = -1.0;
-  for (int bo = bo_max; bo >= 1; --bo) {
-    if (bo < bo_max && ceil_div(na, bo) == ceil_div(na, bo + 1)) continue;   // same block count: skip
-    std::vector<long long> load;
-    deal_block_triples(na, bo, shard_count, &load);
-    long long mx = 0, sum = 0;
-    for (long long l : load) { mx = std::max(mx, l); sum += l; }
-    if (sum == 0) return bo_max;
-    const double imb = (double)mx * shard_count / (double)sum;
-    if (best < 0 || imb < best - 1e-12) { best = imb; best_bo = bo; }
-    if (imb <= 1.03) break;
-    if (ceil_div(na, bo) > 64) break;   // enough block triples (> 45 000): stop searching
-  }
-  return best_bo;
-}
-
-int make_plan(Plan& P, int o, int v, int X, const std::vector<int>& act, const bqc_t_opts* opts) {
-  P.o = o; P.v = v; P.X = X;
-  P.act = act;
-  P.na = (int)act.size();
-  P.Xp = round_up_i(X, 16);
-  P.Kp = round_up_i(v + o, 16);
-  P.nbv = ceil_div(v, kVB);
-  P.fsz = (size_t)P.nbv * P.nbv * P.nbv * (kVB * kVB * kVB);
-  P.slab_elems = (size_t)v * v * P.Kp;
-  P.norbits = (int)((long long)P.nbv * (P.nbv + 1) * (P.nbv + 2) / 6);
-  P.use_t1 = !(opts && (opts->flags & BQC_T_FLAG_NO_T1));
-  P.profile = (opts && (opts->flags & BQC_T_FLAG_PROFILE)) ? 1 : 0;
-  P.shard_count = (opts && opts->shard_count > 0) ? opts->shard_count : 1;
-  P.shard_rank = opts ? opts->shard_rank : 0;
-  P.shard_blocks = (opts && (opts->flags & BQC_T_FLAG_SHARD_BLOCKS)) ? 1 : 0;
-  if (P.shard_rank < 0 || P.shard_rank >= P.shard_count) {
-    set_error(BQC_ERR_INVALID_OPTION, "shard_rank %d outside [0,%d)", P.shard_rank, P.shard_count);
-    return BQC_ERR_INVALID_OPTION;
-  }
-  int bo = opts ? opts->occ_block : 0;
-  if (bo < 0) {
-    set_error(BQC_ERR_INVALID_OPTION, "occ_block %d < 0", bo);
-    return BQC_ERR_INVALID_OPTION;
-  }
-  P.Bo = bo > 0 ? std::min(bo, P.na) : auto_occ_block(P.na, v, P.Kp);
-  if (bo == 0 && P.shard_blocks && P.shard_count > 1) P.Bo = balanced_occ_block(P.na, P.Bo, P.shard_count);
-  P.nblk = ceil_div(P.na, P.Bo);
-  P.nsets = P.nblk == 1 ? 1 : 4;
-  P.nslots = P.nsets * P.Bo;
-  int nbatch = opts ? opts->max_batch : 0;
-  if (nbatch < 0) {
-    set_error(BQC_ERR_INVALID_OPTION, "max_batch %d < 0", nbatch);
-    return BQC_ERR_INVALID_OPTION;
-  }
-  if (nbatch == 0) {
-    const double per = 3.0 * (double)P.fsz * 8.0;
-    nbatch = (int)floor(6.0 * 1073741824.0 / per);
-  }
-  P.nbatch = std::max(1, std::min(nbatch, 1024));
-
-  // upper bounds for the schedule arrays: every active triplet once, + DF tasks
-  size_t ntrip_act = (size_t)P.na * (P.na + 1) * (P.na + 2) / 6;
-  P.max_trips = ntrip_act + 8;
-  P.max_tasks = 3 * ntrip_act + 64 + (size_t)P.na * P.na * 2 + 4 * (size_t)P.na;
-
-  size_t off = 0;
-  auto take = [&](size_t bytes) { size_t r = off; off = round_up(off + bytes, 1024); return r; };
-  P.off_btvv = take((size_t)v * v * P.Xp * 8);
-  P.off_btov = take((size_t)o * v * P.Xp * 8);
-  P.off_btoo = take((size_t)o * o * P.Xp * 8);
-  P.off_btil = take((size_t)P.na * P.na * v * P.Kp * 8);
-  P.off_J = take((size_t)P.na * P.na * v * v * 8);
-  P.off_slabs = take((size_t)P.nslots * P.slab_elems * 8);
-  P.off_F = take((size_t)P.nbatch * 3 * P.fsz * 8);
-  P.off_partial = take((size_t)P.nbatch * P.norbits * 8);
-  P.off_etrip = take(num_triplets(o) * 8);
-  P.off_esum = take(64);
-  P.off_act = take((size_t)P.na * 4);
-  P.off_orbits = take((size_t)P.norbits * 4);
-  P.off_tasks = take(P.max_tasks * sizeof(GemmTask));
-  P.off_trips = take(P.max_trips * sizeof(TripletRec));
-  P.total = off;
-  return BQC_OK;
-}
-
-}  // namespace
 
 // ------------------------------------------------------------------ argument checks (shared with mp2.cu)
 int check_sizes(int o, int v, int X) {
@@ -280,73 +100,10 @@ int check_device() {
 
 namespace {
 
+// caller-space device pointers (never dualised: the packing kernels read them as they are)
 struct Inputs {
   const double *eps_occ, *eps_vir, *t1, *t2, *B_oo, *B_ov, *B_vv;
   const double* f_ov = nullptr;   // optional occupied-virtual Fock block (bqc_t_opts.f_ov)
-};
-
-// ------------------------------------------------------------------ run context
-struct Ctx {
-  Plan P;
-  Inputs in;
-  uint8_t* ws = nullptr;
-  bool own_ws = false;
-  cudaStream_t s_main = nullptr, s_form = nullptr;
-  cudaEvent_t ev_formed[4] = {}, ev_free[4] = {}, ev_fork = nullptr, ev_join = nullptr;
-  bool ev_free_valid[4] = {};
-  int set_block[4] = {-1, -1, -1, -1};
-  // F-GEMM configuration
-  MSegment f_mseg[2];                // row segments of the F GEMM (split_m): main tiles + remainder strip
-  int f_nmseg = 0;
-  NSegment f_seg[2];                 // column segments of the F GEMM (split_n): exact cover of v up to 16
-  int f_nseg = 0;
-  CUtensorMap tm_slab[2], tm_slabT[2], tm_btil[2];
-  // host schedule
-  std::vector<GemmTask> tasks;
-  std::vector<TripletRec> trips;
-  // BQC_T_FLAG_PROFILE: timing events, [3n] before W builder, [3n+1] after it, [3n+2] after the energy kernels
-  std::vector<cudaEvent_t> prof_main;
-  std::vector<cudaEvent_t> prof_form;   // [2n], [2n+1] around each slab-block formation
-  cudaEvent_t prof_begin = nullptr, prof_prepared = nullptr, prof_end = nullptr;
-  int prof_mark(std::vector<cudaEvent_t>& v, cudaStream_t s) {
-    cudaEvent_t e;
-    BQC_CUDA_OK(cudaEventCreate(&e));
-    v.push_back(e);
-    BQC_CUDA_OK(cudaEventRecord(e, s));
-    return BQC_OK;
-  }
-
-  double* d(size_t off) const { return reinterpret_cast<double*>(ws + off); }
-  double* btvv() const { return d(P.off_btvv); }
-  double* btov() const { return d(P.off_btov); }
-  double* btoo() const { return d(P.off_btoo); }
-  double* btil() const { return d(P.off_btil); }
-  double* J() const { return d(P.off_J); }
-  double* slabs() const { return d(P.off_slabs); }
-  double* F() const { return d(P.off_F); }
-  double* partial() const { return d(P.off_partial); }
-  double* etrip() const { return d(P.off_etrip); }
-  double* esum() const { return d(P.off_esum); }
-  int* act_dev() const { return reinterpret_cast<int*>(ws + P.off_act); }
-  int* orbits_dev() const { return reinterpret_cast<int*>(ws + P.off_orbits); }
-  GemmTask* tasks_dev() const { return reinterpret_cast<GemmTask*>(ws + P.off_tasks); }
-  TripletRec* trips_dev() const { return reinterpret_cast<TripletRec*>(ws + P.off_trips); }
-
-  ~Ctx() {
-    for (cudaEvent_t e : prof_main) cudaEventDestroy(e);
-    for (cudaEvent_t e : prof_form) cudaEventDestroy(e);
-    if (prof_begin) cudaEventDestroy(prof_begin);
-    if (prof_prepared) cudaEventDestroy(prof_prepared);
-    if (prof_end) cudaEventDestroy(prof_end);
-    for (int s = 0; s < 4; ++s) {
-      if (ev_formed[s]) cudaEventDestroy(ev_formed[s]);
-      if (ev_free[s]) cudaEventDestroy(ev_free[s]);
-    }
-    if (ev_fork) cudaEventDestroy(ev_fork);
-    if (ev_join) cudaEventDestroy(ev_join);
-    if (s_form) cudaStreamDestroy(s_form);
-    if (own_ws && ws) cudaFree(ws);
-  }
 };
 
 struct Run { int pos0, orb0, len; };   // a run of consecutive orbitals inside the active list
@@ -360,11 +117,6 @@ std::vector<Run> runs_of(const std::vector<int>& act, int p0, int p1) {
     p = q;
   }
   return r;
-}
-
-size_t push_task(Ctx& c, const GemmTask& t) {
-  c.tasks.push_back(t);
-  return c.tasks.size() - 1;
 }
 
 GemmTask single_term_task(long long c_off) {
@@ -388,16 +140,319 @@ struct DfGemm {
   const double* B; long long b_rows;        // B tensor [b_rows][Xp]
   int m1_base, m1_ext, m2_ext;
   int n_base; long long n_ext;
-  long long c_off, sM1, sM2, sN1, sN2; int n2_ext;
-  double* C;
+  long long sM1, sM2, sN1, sN2; int n2_ext;
+  double* C;                                // output base (element (0,0,0) of this GEMM)
 };
 
-int run_df_gemm(Ctx& c, const DfGemm& g, size_t task_slot, cudaStream_t s) {
-  const Plan& P = c.P;
-  if (task_slot >= c.tasks.size() || c.tasks[task_slot].nterms != 1 || c.tasks[task_slot].c_off != g.c_off) {
-    set_error(BQC_ERR_CUDA, "internal: DF task slot %zu does not match its launch", task_slot);
-    return BQC_ERR_CUDA;
+struct Action {
+  enum Kind { FORM, PAIR, TRIPLE } kind;
+  int set, block;                 // FORM: slab set <- block.  PAIR: first set / block (z).  TRIPLE: unused
+  int set2, block2;               // PAIR: second set / block (y)
+  int need_j, need_panel;         // PAIR: also form J; (re)build the K-major panel of block2
+  int I, J, K, sJ, sK;            // TRIPLE: the block triple and the slab sets of its J and K blocks (I: set 0)
+};
+
+// ------------------------------------------------------------------ the engine
+// Everything that does not depend on the values of the inputs: plan, workspace, helper stream, events,
+// tensor maps and the host-built schedule.  Reused across calls with the same sizes/options (see engine_for).
+struct Engine {
+  Plan P;
+  int nocc = 0, nvir = 0, naux = 0;   // caller space
+  bqc_t_opts key_opts;                // options the engine was built for (f_ov reduced to NULL / non-NULL)
+  void* key_ws = nullptr;             // caller workspace the engine was built on (NULL: owns its own)
+  size_t key_ws_bytes = 0;
+  int device = -1;
+  Inputs in;
+  uint8_t* ws = nullptr;
+  bool own_ws = false;
+  cudaStream_t s_main = nullptr, s_form = nullptr;
+  cudaEvent_t ev_formed[4] = {}, ev_free[4] = {}, ev_fork = nullptr, ev_join = nullptr;
+  bool ev_free_valid[4] = {};
+  // F-GEMM configuration
+  MSegment f_mseg[2];                // row segments of the F GEMM (split_m): main tiles + remainder strip
+  int f_nmseg = 0;
+  NSegment f_seg[2];                 // column segments of the F GEMM (split_n): exact cover of v up to 16
+  int f_nseg = 0;
+  CUtensorMap tm_slab[2], tm_slabT[2], tm_btil[2];
+  // host schedule: the action list (slab-set / pair-block formations and block triples, in order); the
+  // triplet records and F-GEMM tasks of a block triple are generated when it is reached, into one of two
+  // pinned chunks, and uploaded into the matching device chunk (so nothing of size #triplets lives anywhere)
+  std::vector<int> orbits;
+  std::vector<Action> actions;
+  std::vector<int> bt_owner;         // BQC_T_FLAG_SHARD_BLOCKS: owner of every block triple
+  size_t ncompute = 0;               // W-builder launches of the whole schedule
+  GemmTask df_task;                  // the one task of every DF GEMM (single term, c_off 0)
+  uint8_t* pinned = nullptr;         // 2 chunks: [chunk_trips TripletRec][3 chunk_trips GemmTask]
+  cudaEvent_t ev_up[2] = {};         // upload of chunk b has executed: its pinned half may be rewritten
+  bool ev_up_valid[2] = {};
+  int chunk_next = 0;
+  // BQC_T_FLAG_PROFILE: timing events (pooled, reused across calls)
+  std::vector<cudaEvent_t> ev_pool;
+  size_t ev_used = 0;
+  std::vector<cudaEvent_t> prof_main;   // [3n] before W builder, [3n+1] after it, [3n+2] after the energy kernels
+  std::vector<cudaEvent_t> prof_form;   // [2n], [2n+1] around each slab-block / pair-block formation
+  cudaEvent_t prof_begin = nullptr, prof_prepared = nullptr, prof_end = nullptr;
+
+  int prof_mark(std::vector<cudaEvent_t>& v, cudaStream_t s) {
+    if (ev_used == ev_pool.size()) {
+      cudaEvent_t e;
+      BQC_CUDA_OK(cudaEventCreate(&e));
+      ev_pool.push_back(e);
+    }
+    cudaEvent_t e = ev_pool[ev_used++];
+    v.push_back(e);
+    BQC_CUDA_OK(cudaEventRecord(e, s));
+    return BQC_OK;
   }
+
+  double* d(size_t off) const { return reinterpret_cast<double*>(ws + off); }
+  double* btvv() const { return d(P.off_btvv); }
+  double* btov() const { return d(P.off_btov); }
+  double* panel() const { return d(P.off_panel); }
+  double* btil() const { return d(P.off_btil); }
+  double* J() const { return d(P.off_J); }
+  double* slabs() const { return d(P.off_slabs); }
+  double* F() const { return d(P.off_F); }
+  double* partial() const { return d(P.off_partial); }
+  double* etrip() const { return d(P.off_etrip); }
+  double* esum() const { return d(P.off_esum); }
+  int* orbits_dev() const { return reinterpret_cast<int*>(ws + P.off_orbits); }
+  GemmTask* df_task_dev() const { return reinterpret_cast<GemmTask*>(ws + P.off_tasks); }
+  // device chunk b: F tasks follow the DF task slot(s) at off_tasks
+  GemmTask* tasks_dev(int b) const { return df_task_dev() + 8 + (size_t)b * 3 * P.chunk_trips; }
+  TripletRec* trips_dev(int b) const { return reinterpret_cast<TripletRec*>(ws + P.off_trips) + (size_t)b * P.chunk_trips; }
+  size_t pinned_chunk_bytes() const { return P.chunk_trips * (sizeof(TripletRec) + 3 * sizeof(GemmTask)); }
+  TripletRec* trips_host(int b) const { return reinterpret_cast<TripletRec*>(pinned + (size_t)b * pinned_chunk_bytes()); }
+  GemmTask* tasks_host(int b) const { return reinterpret_cast<GemmTask*>(trips_host(b) + P.chunk_trips); }
+  // pipeline-space views of the small inputs (dual copies live in the workspace)
+  const double* eps_o() const { return P.dual ? d(P.off_small + P.small_eo) : in.eps_occ; }
+  const double* eps_v() const { return P.dual ? d(P.off_small + P.small_ev) : in.eps_vir; }
+  const double* t1p() const { return P.dual ? d(P.off_small + P.small_t1) : in.t1; }
+  const double* fp() const { return !in.f_ov ? nullptr : (P.dual ? d(P.off_small + P.small_f) : in.f_ov); }
+  // pipeline-space DF blocks: inner-inner, outer-outer (the caller's arrays, Q-major)
+  const double* B_inner() const { return P.dual ? in.B_oo : in.B_vv; }
+  const double* B_outer() const { return P.dual ? in.B_vv : in.B_oo; }
+
+  int block_begin(int b) const { return b * P.Bo; }
+  int block_end(int b) const { return std::min(P.na, (b + 1) * P.Bo); }
+  int slot_of(int pos, int set, int block) const { return set * P.Bo + (pos - block_begin(block)); }
+
+  int init(int nocc_, int nvir_, int naux_, const bqc_t_opts* opts, void* workspace, size_t workspace_bytes,
+           const std::vector<int>* act_override);
+  int build_schedule();
+  int run_df_gemm(const DfGemm& g, cudaStream_t s);
+  int launch_f_gemm(GemmParams prm, cudaStream_t s);
+  int prepare(cudaStream_t s);
+  int exec_form(int set, int block, cudaStream_t s);
+  int exec_pair(const Action& a, cudaStream_t s);
+  size_t list_triple(const Action& a, TripletRec* trips, GemmTask* tasks) const;
+  int exec_triple(const Action& a, cudaStream_t s);
+  int exec_compute(int chunk, size_t trip0, size_t ntrip, cudaStream_t s);
+  int execute();
+  int run(const Inputs& inputs, double* e_total_host, double* e_triplet_dev, cudaStream_t stream);
+
+  ~Engine() {
+    for (cudaEvent_t e : ev_pool) cudaEventDestroy(e);
+    if (prof_begin) cudaEventDestroy(prof_begin);
+    if (prof_prepared) cudaEventDestroy(prof_prepared);
+    if (prof_end) cudaEventDestroy(prof_end);
+    for (int s = 0; s < 4; ++s) {
+      if (ev_formed[s]) cudaEventDestroy(ev_formed[s]);
+      if (ev_free[s]) cudaEventDestroy(ev_free[s]);
+    }
+    if (ev_fork) cudaEventDestroy(ev_fork);
+    if (ev_join) cudaEventDestroy(ev_join);
+    for (int b = 0; b < 2; ++b)
+      if (ev_up[b]) cudaEventDestroy(ev_up[b]);
+    if (s_form) cudaStreamDestroy(s_form);
+    if (pinned) cudaFreeHost(pinned);
+    if (own_ws && ws) cudaFree(ws);
+  }
+};
+
+int Engine::init(int nocc_, int nvir_, int naux_, const bqc_t_opts* opts, void* workspace,
+                 size_t workspace_bytes, const std::vector<int>* act_override) {
+  nocc = nocc_; nvir = nvir_; naux = naux_;
+  memset(&key_opts, 0, sizeof(key_opts));
+  if (opts) key_opts = *opts;
+  key_ws = workspace;
+  key_ws_bytes = workspace_bytes;
+  BQC_CUDA_OK(cudaGetDevice(&device));
+  if (act_override)
+    BQC_TRY(make_plan(P, nocc, nvir, naux, false, *act_override, opts));
+  else
+    BQC_TRY(make_plan_for(P, nocc, nvir, naux, opts));
+  if (workspace) {
+    if (workspace_bytes < P.total || (reinterpret_cast<uintptr_t>(workspace) & 255)) {
+      set_error(BQC_ERR_WORKSPACE, "workspace of %zu bytes (need %zu, 256-byte aligned; largest buffer: %s, %zu bytes)",
+                workspace_bytes, P.total, P.biggest_name, P.biggest_bytes);
+      return BQC_ERR_WORKSPACE;
+    }
+    ws = static_cast<uint8_t*>(workspace);
+  } else {
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, P.total);
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      size_t fr = 0, tot = 0;
+      cudaMemGetInfo(&fr, &tot);
+      set_error(BQC_ERR_WORKSPACE,
+                "cudaMalloc of %zu workspace bytes failed (%s; %zu bytes free); largest buffer: %s, %zu bytes — "
+                "lower opts.workspace_gib or opts.occ_block / max_batch",
+                P.total, cudaGetErrorString(e), fr, P.biggest_name, P.biggest_bytes);
+      return BQC_ERR_WORKSPACE;
+    }
+    ws = static_cast<uint8_t*>(p);
+    own_ws = true;
+  }
+  BQC_CUDA_OK(cudaStreamCreateWithFlags(&s_form, cudaStreamNonBlocking));
+  for (int s = 0; s < 4; ++s) {
+    BQC_CUDA_OK(cudaEventCreateWithFlags(&ev_formed[s], cudaEventDisableTiming));
+    BQC_CUDA_OK(cudaEventCreateWithFlags(&ev_free[s], cudaEventDisableTiming));
+  }
+  BQC_CUDA_OK(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
+  BQC_CUDA_OK(cudaEventCreateWithFlags(&ev_join, cudaEventDisableTiming));
+  for (int b = 0; b < 2; ++b) BQC_CUDA_OK(cudaEventCreateWithFlags(&ev_up[b], cudaEventDisableTiming));
+  BQC_CUDA_OK(cudaMallocHost(&pinned, 2 * pinned_chunk_bytes()));
+  df_task = single_term_task(0);
+
+  const int v = P.v;
+  f_nmseg = split_m(v, v, f_mseg);
+  f_nseg = split_n(v, f_seg);
+  for (int m = 0; m < f_nmseg; ++m) {
+    const int tq = 1 << f_mseg[m].tq_log2;
+    BQC_TRY(tmap(&tm_slab[m], slabs(), P.Kp, v, v, P.nslots, tq, f_mseg[m].tp));
+    BQC_TRY(tmap(&tm_slabT[m], slabs(), P.Kp, v, v, P.nslots, 1, tq));
+  }
+  for (int n = 0; n < f_nseg; ++n)
+    BQC_TRY(tmap(&tm_btil[n], btil(), P.Kp, v, (unsigned long long)P.nslots * P.nslots, 1, gemm_bn(f_seg[n].nf), 1));
+  // orbit table A <= B <= C of 8-blocks of the inner index
+  orbits.reserve(P.norbits);
+  for (int A = 0; A < P.nbv; ++A)
+    for (int B = A; B < P.nbv; ++B)
+      for (int C = B; C < P.nbv; ++C) orbits.push_back(A | (B << 10) | (C << 20));
+  return build_schedule();
+}
+
+// Triplet records (and, if tasks != NULL, the three F-GEMM tasks of each) of block triple `a` owned by this
+// shard, in loop order.  Returns their number.
+size_t Engine::list_triple(const Action& a, TripletRec* trips, GemmTask* tasks) const {
+  size_t n = 0;
+  for (int pi = block_begin(a.I); pi < block_end(a.I); ++pi)
+    for (int pj = std::max(pi, block_begin(a.J)); pj < block_end(a.J); ++pj)
+      for (int pk = std::max(pj, block_begin(a.K)); pk < block_end(a.K); ++pk) {
+        if (pi == pj && pj == pk) continue;   // g(i,i,i) = 0 exactly
+        TripletRec t;
+        t.i = P.act[pi]; t.j = P.act[pj]; t.k = P.act[pk];
+        t.pi = slot_of(pi, 0, a.I); t.pj = slot_of(pj, a.sJ, a.J); t.pk = slot_of(pk, a.sK, a.K);
+        t.index = (long long)triplet_index(P.o, t.i, t.j, t.k);
+        if (!P.shard_blocks && (int)(t.index % P.shard_count) != P.shard_rank) continue;
+        if (trips) trips[n] = t;
+        if (tasks) {
+          const size_t in_batch = n % (size_t)P.nbatch;   // F arrays are indexed within a W-builder launch
+          auto pair = [&](int sz, int sy) { return sz * P.nslots + sy; };
+          // F(x,y,z): term0 = (I~_x, canonical rows, B~_zy), term1 = (I~_y, transposed rows, B~_zx)
+          auto f_task = [&](int sx, int sy, int sz, int cls) {
+            GemmTask& g = tasks[3 * n + cls];
+            memset(&g, 0, sizeof(g));
+            g.nterms = 2;
+            g.term[0].a_idx = sx; g.term[0].a_transposed = 0; g.term[0].b_idx = pair(sz, sy);
+            g.term[1].a_idx = sy; g.term[1].a_transposed = 1; g.term[1].b_idx = pair(sz, sx);
+            g.c_off = (long long)((in_batch * 3 + cls) * P.fsz);
+          };
+          f_task(t.pi, t.pj, t.pk, 0);   // F(i,j,k)
+          f_task(t.pi, t.pk, t.pj, 1);   // F(i,k,j)
+          f_task(t.pj, t.pk, t.pi, 2);   // F(j,k,i)
+        }
+        ++n;
+      }
+  return n;
+}
+
+int Engine::build_schedule() {
+  const int Bo = P.Bo;
+  actions.clear();
+  ncompute = 0;
+
+  // ---- block triples I <= J <= K with the slot-set protocol: I -> set 0, J -> set 1, K -> sets 2/3
+  int set_block[4] = {-1, -1, -1, -1};
+  struct PairTag { int bz = -1, by = -1, has_j = 0; } tag[4][4];
+  int panel_block = -1;
+  int kflip = 0;
+  auto acquire = [&](int set, int block) {
+    if (set_block[set] == block) return;
+    Action a;
+    memset(&a, 0, sizeof(a));
+    a.kind = Action::FORM; a.set = set; a.block = block;
+    actions.push_back(a);
+    set_block[set] = block;
+  };
+  const bool single_run_blocks = (P.nruns == 1);
+
+  long long block_triple = -1;
+  bt_owner.clear();
+  if (P.shard_blocks) bt_owner = deal_block_triples(P.na, Bo, P.shard_count);
+  for (int I = 0; I < P.nblk; ++I) {
+    for (int Jb = I; Jb < P.nblk; ++Jb) {
+      const int sJ = (Jb == I) ? 0 : 1;
+      for (int K = Jb; K < P.nblk; ++K) {
+        ++block_triple;
+        // BQC_T_FLAG_SHARD_BLOCKS: whole block triples are dealt to the shards, so a shard forms only the
+        // slabs of its own block triples; otherwise every shard owns some triplets of every block triple
+        if (P.shard_blocks && bt_owner[(size_t)block_triple] != P.shard_rank) continue;
+        int sK = sJ;
+        if (K != Jb) sK = (set_block[2] == K) ? 2 : (set_block[3] == K ? 3 : 2 + (kflip & 1));
+        Action t;
+        memset(&t, 0, sizeof(t));
+        t.kind = Action::TRIPLE;
+        t.I = I; t.J = Jb; t.K = K; t.sJ = sJ; t.sK = sK;
+        // triplets of this block triple owned by this shard (every one, unless the per-triplet modulo shards)
+        const size_t ntr = (P.shard_count > 1 && !P.shard_blocks) ? list_triple(t, nullptr, nullptr)
+                                                                  : (size_t)block_triple_work(P.na, Bo, I, Jb, K);
+        if (ntr == 0) continue;
+        if (ntr > P.chunk_trips) {
+          set_error(BQC_ERR_WORKSPACE, "internal: block triple of %zu triplets exceeds the chunk of %zu", ntr,
+                    P.chunk_trips);
+          return BQC_ERR_WORKSPACE;
+        }
+        if (K != Jb && sK >= 2 && set_block[sK] != K) ++kflip;
+        // slabs are formed only for block triples that have work (the acquire calls are idempotent)
+        acquire(0, I);
+        if (Jb != I) acquire(1, Jb);
+        if (K != Jb) acquire(sK, K);
+        // B~ / J pair blocks of the ordered set pairs this block triple touches
+        const int sets[3] = {0, sJ, sK}, blks[3] = {I, Jb, K};
+        for (int p = 0; p < 3; ++p)
+          for (int q = 0; q < 3; ++q) {
+            if (p == q) continue;
+            const int sz = sets[p], sy = sets[q];
+            const int want_j = (p < q) ? 1 : 0;   // J_ij, J_ik, J_jk: the earlier orbital first
+            PairTag& tg = tag[sz][sy];
+            if (tg.bz == blks[p] && tg.by == blks[q] && (tg.has_j || !want_j)) continue;
+            // when the same set pair comes again in this loop as an (earlier, later) pair it wants J: form it now
+            int need_j = want_j;
+            for (int p2 = 0; p2 < 3; ++p2)
+              for (int q2 = p2 + 1; q2 < 3; ++q2)
+                if (sets[p2] == sz && sets[q2] == sy) need_j = 1;
+            Action a;
+            memset(&a, 0, sizeof(a));
+            a.kind = Action::PAIR;
+            a.set = sz; a.block = blks[p]; a.set2 = sy; a.block2 = blks[q];
+            a.need_j = need_j;
+            a.need_panel = !(single_run_blocks && panel_block == blks[q]);
+            panel_block = single_run_blocks ? blks[q] : -1;
+            actions.push_back(a);
+            tg.bz = blks[p]; tg.by = blks[q]; tg.has_j = need_j;
+          }
+        actions.push_back(t);
+        ncompute += (ntr + P.nbatch - 1) / P.nbatch;
+      }
+    }
+  }
+  return BQC_OK;
+}
+
+int Engine::run_df_gemm(const DfGemm& g, cudaStream_t s) {
   int tp, tql;
   choose_m_tile(g.m1_ext, g.m2_ext, &tp, &tql);
   const int tq = 1 << tql;
@@ -418,346 +473,195 @@ int run_df_gemm(Ctx& c, const DfGemm& g, size_t task_slot, cudaStream_t s) {
   prm.out_mode = 0;
   prm.n2_ext = g.n2_ext;
   prm.sM1 = g.sM1; prm.sM2 = g.sM2; prm.sN1 = g.sN1; prm.sN2 = g.sN2;
-  prm.tasks = c.tasks_dev() + task_slot;
+  prm.tasks = df_task_dev();   // single term, a_idx = b_idx = 0, c_off = 0
   prm.C = g.C;
   return launch_gemm_nt(nf, tA, tA, tB, prm, s);
 }
 
-// ------------------------------------------------------------------ the pipeline
-struct Action {
-  enum Kind { FORM, COMPUTE } kind;
-  int set, block;                 // FORM
-  size_t trip0, ntrip, task0;     // COMPUTE (indices into the schedule arrays)
-  int sets_used[3];
-};
-
-struct Pipeline {
-  Ctx c;
-  std::vector<Action> actions;
-  std::vector<size_t> form_task_slot;   // per FORM action run: task slots (one per run)
-
-  int setup(int o, int v, int X, const Inputs& in, const std::vector<int>& act, const bqc_t_opts* opts,
-            void* workspace, size_t workspace_bytes, cudaStream_t stream);
-  int prepare();                          // repack inputs, B~, J, zero-fills
-  int form_block(int set, int block, cudaStream_t s);
-  int build_schedule();
-  int compute(const Action& a);
-  int execute();
-  int block_begin(int b) const { return b * c.P.Bo; }
-  int block_end(int b) const { return std::min(c.P.na, (b + 1) * c.P.Bo); }
-};
-
-int Pipeline::setup(int o, int v, int X, const Inputs& in, const std::vector<int>& act,
-                    const bqc_t_opts* opts, void* workspace, size_t workspace_bytes, cudaStream_t stream) {
-  BQC_TRY(make_plan(c.P, o, v, X, act, opts));
-  c.in = in;
-  c.s_main = stream;
-  if (workspace) {
-    if (workspace_bytes < c.P.total || (reinterpret_cast<uintptr_t>(workspace) & 255)) {
-      set_error(BQC_ERR_WORKSPACE, "workspace of %zu bytes (need %zu, 256-byte aligned)", workspace_bytes,
-                c.P.total);
-      return BQC_ERR_WORKSPACE;
-    }
-    c.ws = static_cast<uint8_t*>(workspace);
-  } else {
-    void* p = nullptr;
-    cudaError_t e = cudaMalloc(&p, c.P.total);
-    if (e != cudaSuccess) {
-      cudaGetLastError();
-      set_error(BQC_ERR_WORKSPACE, "cudaMalloc of %zu workspace bytes failed: %s", c.P.total,
-                cudaGetErrorString(e));
-      return BQC_ERR_WORKSPACE;
-    }
-    c.ws = static_cast<uint8_t*>(p);
-    c.own_ws = true;
-  }
-  BQC_CUDA_OK(cudaStreamCreateWithFlags(&c.s_form, cudaStreamNonBlocking));
-  for (int s = 0; s < 4; ++s) {
-    BQC_CUDA_OK(cudaEventCreateWithFlags(&c.ev_formed[s], cudaEventDisableTiming));
-    BQC_CUDA_OK(cudaEventCreateWithFlags(&c.ev_free[s], cudaEventDisableTiming));
-  }
-  BQC_CUDA_OK(cudaEventCreateWithFlags(&c.ev_fork, cudaEventDisableTiming));
-  BQC_CUDA_OK(cudaEventCreateWithFlags(&c.ev_join, cudaEventDisableTiming));
-
-  const Plan& P = c.P;
-  c.f_nmseg = split_m(v, v, c.f_mseg);
-  c.f_nseg = split_n(v, c.f_seg);
-  for (int m = 0; m < c.f_nmseg; ++m) {
-    const int tq = 1 << c.f_mseg[m].tq_log2;
-    BQC_TRY(tmap(&c.tm_slab[m], c.slabs(), P.Kp, v, v, P.nslots, tq, c.f_mseg[m].tp));
-    BQC_TRY(tmap(&c.tm_slabT[m], c.slabs(), P.Kp, v, v, P.nslots, 1, tq));
-  }
-  for (int n = 0; n < c.f_nseg; ++n)
-    BQC_TRY(tmap(&c.tm_btil[n], c.btil(), P.Kp, v, (unsigned long long)P.na * P.na, 1, gemm_bn(c.f_seg[n].nf), 1));
-  return BQC_OK;
-}
-
 // The W-builder GEMM of `prm.ntasks` tasks: one launch per (row segment, column segment).
-int launch_f_gemm(Ctx& c, GemmParams prm, cudaStream_t s) {
-  const int v = c.P.v;
+int Engine::launch_f_gemm(GemmParams prm, cudaStream_t s) {
+  const int v = P.v;
   prm.m1_ext = v; prm.m2_ext = v; prm.n_ext = v;
-  prm.kiters = c.P.Kp / kBK;
+  prm.kiters = P.Kp / kBK;
   prm.out_mode = 1;
-  prm.nbv = c.P.nbv;
+  prm.nbv = P.nbv;
   prm.n2_ext = 1;
-  for (int m = 0; m < c.f_nmseg; ++m) {
-    const MSegment& ms = c.f_mseg[m];
+  for (int m = 0; m < f_nmseg; ++m) {
+    const MSegment& ms = f_mseg[m];
     prm.tp = ms.tp; prm.tq_log2 = ms.tq_log2;
     prm.tiles_m1 = ms.tiles_m1;
     prm.tiles_m2 = ceil_div(v, 1 << ms.tq_log2);
     prm.m1_base = prm.m1_out = ms.m1_0;
-    for (int n = 0; n < c.f_nseg; ++n) {
-      prm.tiles_n = c.f_seg[n].ntiles;
-      prm.n_base = prm.n_out = c.f_seg[n].n0;
-      BQC_TRY(launch_gemm_nt(c.f_seg[n].nf, c.tm_slab[m], c.tm_slabT[m], c.tm_btil[n], prm, s));
+    for (int n = 0; n < f_nseg; ++n) {
+      prm.tiles_n = f_seg[n].ntiles;
+      prm.n_base = prm.n_out = f_seg[n].n0;
+      BQC_TRY(launch_gemm_nt(f_seg[n].nf, tm_slab[m], tm_slabT[m], tm_btil[n], prm, s));
     }
   }
   return BQC_OK;
 }
 
-int Pipeline::prepare() {
-  const Plan& P = c.P;
-  cudaStream_t s = c.s_main;
-  const int o = P.o, v = P.v, X = P.X, na = P.na;
-  // K-major copies of the DF factors: Bt[r][Q] = B[Q][r]
-  BQC_TRY(launch_transpose_pad(c.in.B_vv, c.btvv(), X, v * v, P.Xp, s));
-  BQC_TRY(launch_transpose_pad(c.in.B_ov, c.btov(), X, o * v, P.Xp, s));
-  BQC_TRY(launch_transpose_pad(c.in.B_oo, c.btoo(), X, o * o, P.Xp, s));
-  // zero fills: K padding of B~ and slabs, pad blocks of F, per-triplet energies
-  BQC_CUDA_OK(cudaMemsetAsync(c.btil(), 0, (size_t)na * na * v * P.Kp * 8, s));
-  BQC_CUDA_OK(cudaMemsetAsync(c.slabs(), 0, (size_t)P.nslots * P.slab_elems * 8, s));
-  BQC_CUDA_OK(cudaMemsetAsync(c.F(), 0, (size_t)P.nbatch * 3 * P.fsz * 8, s));
-  BQC_CUDA_OK(cudaMemsetAsync(c.etrip(), 0, num_triplets(o) * 8, s));
-  BQC_CUDA_OK(cudaMemcpyAsync(c.act_dev(), P.act.data(), (size_t)na * 4, cudaMemcpyHostToDevice, s));
-  // orbit table A <= B <= C
-  {
-    std::vector<int> orb;
-    orb.reserve(P.norbits);
-    for (int A = 0; A < P.nbv; ++A)
-      for (int B = A; B < P.nbv; ++B)
-        for (int C = B; C < P.nbv; ++C) orb.push_back(A | (B << 10) | (C << 20));
-    BQC_CUDA_OK(cudaMemcpyAsync(c.orbits_dev(), orb.data(), orb.size() * 4, cudaMemcpyHostToDevice, s));
-    BQC_CUDA_OK(cudaStreamSynchronize(s));   // `orb` goes out of scope
+// Per-call set-up on the main stream: dual views of the small inputs, K-major copies of the DF factors the
+// slab former reads, zero K-padding, the static tables.  Nothing here synchronises the host: the host
+// vectors that are uploaded live in the engine.
+int Engine::prepare(cudaStream_t s) {
+  const int o = P.o, v = P.v, X = P.X;
+  if (P.dual) {
+    // eps_occ' = -eps_vir, eps_vir' = -eps_occ, t1'[a,i] = t1[i,a], f'[a,i] = -f[i,a]
+    BQC_TRY(launch_transpose_scale(in.eps_vir, d(P.off_small + P.small_eo), 1, 1, o, -1.0, s));
+    BQC_TRY(launch_transpose_scale(in.eps_occ, d(P.off_small + P.small_ev), 1, 1, v, -1.0, s));
+    BQC_TRY(launch_transpose_scale(in.t1, d(P.off_small + P.small_t1), 1, v, o, 1.0, s));
+    if (in.f_ov) BQC_TRY(launch_transpose_scale(in.f_ov, d(P.off_small + P.small_f), 1, v, o, -1.0, s));
   }
-  // the whole schedule (GEMM tasks + triplet records) goes up once
-  if (c.tasks.size() > P.max_tasks || c.trips.size() > P.max_trips) {
-    set_error(BQC_ERR_WORKSPACE, "internal: schedule arrays overflow (%zu/%zu tasks, %zu/%zu triplets)",
-              c.tasks.size(), P.max_tasks, c.trips.size(), P.max_trips);
-    return BQC_ERR_WORKSPACE;
+  // K-major copies: Bt_vv[(q,d)][Q] (inner-inner block), Bt_ov[(x,p)][Q] (outer x, inner p)
+  BQC_TRY(launch_transpose_pad(B_inner(), (long long)v * v, 0, (long long)v * v, btvv(), X, P.Xp, 0, 0, s));
+  if (!P.dual)
+    BQC_TRY(launch_transpose_pad(in.B_ov, (long long)o * v, 0, (long long)o * v, btov(), X, P.Xp, 0, 0, s));
+  else   // the caller's B_ov[Q][i][a] has the inner index first: pair-transposed rows
+    BQC_TRY(launch_transpose_pad(in.B_ov, (long long)o * v, 0, (long long)o * v, btov(), X, P.Xp, o, v, s));
+  // zero fills: the K padding columns [v+o, Kp) of B~ and of the slabs (nobody else writes them), e_ijk
+  if (P.Kp > v + o) {
+    const size_t w = (size_t)(P.Kp - v - o) * 8, pitch = (size_t)P.Kp * 8;
+    BQC_CUDA_OK(cudaMemset2DAsync(btil() + (v + o), pitch, 0, w, (size_t)P.nslots * P.nslots * v, s));
+    BQC_CUDA_OK(cudaMemset2DAsync(slabs() + (v + o), pitch, 0, w, (size_t)P.nslots * v * v, s));
   }
-  if (!c.tasks.empty())
-    BQC_CUDA_OK(cudaMemcpyAsync(c.tasks_dev(), c.tasks.data(), c.tasks.size() * sizeof(GemmTask),
-                                cudaMemcpyHostToDevice, s));
-  if (!c.trips.empty())
-    BQC_CUDA_OK(cudaMemcpyAsync(c.trips_dev(), c.trips.data(), c.trips.size() * sizeof(TripletRec),
-                                cudaMemcpyHostToDevice, s));
-
-  // B~ particle columns: t2 rows
-  BQC_TRY(launch_btilde_t2(c.in.t2, c.btil(), o, v, c.act_dev(), na, P.Kp, s));
-  // B~ hole columns (z r|y l) and J_xy[u,w] = (x u|y w), one GEMM per pair of contiguous runs
-  const std::vector<Run> runs = runs_of(P.act, 0, na);
-  size_t slot = 0;   // DF tasks occupy the first slots of the task array (see build_schedule)
-  for (const Run& rz : runs)
-    for (const Run& ry : runs) {
-      DfGemm g;
-      g.A = c.btov(); g.a_d1 = v; g.a_d2 = o;
-      g.B = c.btoo(); g.b_rows = (long long)o * o;
-      g.m1_base = rz.orb0; g.m1_ext = rz.len; g.m2_ext = v;
-      g.n_base = ry.orb0 * o; g.n_ext = (long long)ry.len * o;
-      g.c_off = ((long long)rz.pos0 * na + ry.pos0) * v * P.Kp + v;
-      g.sM1 = (long long)na * v * P.Kp; g.sM2 = P.Kp; g.sN1 = (long long)v * P.Kp; g.sN2 = 1; g.n2_ext = o;
-      g.C = c.btil();
-      BQC_TRY(run_df_gemm(c, g, slot++, s));
-      DfGemm j;
-      j.A = c.btov(); j.a_d1 = v; j.a_d2 = o;
-      j.B = c.btov(); j.b_rows = (long long)o * v;
-      j.m1_base = rz.orb0; j.m1_ext = rz.len; j.m2_ext = v;
-      j.n_base = ry.orb0 * v; j.n_ext = (long long)ry.len * v;
-      j.c_off = ((long long)rz.pos0 * na + ry.pos0) * v * v;
-      j.sM1 = (long long)na * v * v; j.sM2 = v; j.sN1 = (long long)v * v; j.sN2 = 1; j.n2_ext = v;
-      j.C = c.J();
-      BQC_TRY(run_df_gemm(c, j, slot++, s));
-    }
+  BQC_CUDA_OK(cudaMemsetAsync(etrip(), 0, num_triplets(o) * 8, s));
+  // the static tables: orbit table and the DF task (host copies live in the engine; the schedule chunks follow
+  // block triple by block triple, see exec_triple)
+  BQC_CUDA_OK(cudaMemcpyAsync(orbits_dev(), orbits.data(), orbits.size() * 4, cudaMemcpyHostToDevice, s));
+  BQC_CUDA_OK(cudaMemcpyAsync(df_task_dev(), &df_task, sizeof(GemmTask), cudaMemcpyHostToDevice, s));
   // the former stream starts after the repacked inputs exist
-  BQC_CUDA_OK(cudaEventRecord(c.ev_fork, s));
-  BQC_CUDA_OK(cudaStreamWaitEvent(c.s_form, c.ev_fork, 0));
+  BQC_CUDA_OK(cudaEventRecord(ev_fork, s));
+  BQC_CUDA_OK(cudaStreamWaitEvent(s_form, ev_fork, 0));
+  for (int n = 0; n < 4; ++n) ev_free_valid[n] = false;
   return BQC_OK;
 }
 
-// Augmented slabs of one occupied block into slot set `set` (row a1 + hole columns).
-int Pipeline::form_block(int set, int block, cudaStream_t s) {
-  const Plan& P = c.P;
+// Augmented slabs of one outer block into slot set `set` (row a1 + hole columns).
+int Engine::exec_form(int set, int block, cudaStream_t s) {
   const int v = P.v;
   const int p0 = block_begin(block), p1 = block_end(block);
   for (const Run& r : runs_of(P.act, p0, p1)) {
-    const int slot0 = set * P.Bo + (r.pos0 - p0);
+    const int slot0 = slot_of(r.pos0, set, block);
     DfGemm g;
-    g.A = c.btvv(); g.a_d1 = v; g.a_d2 = v;             // rows (m1 = q, m2 = d)
-    g.B = c.btov(); g.b_rows = (long long)P.o * v;      // rows n = (x, p)
+    g.A = btvv(); g.a_d1 = v; g.a_d2 = v;               // rows (m1 = q, m2 = d)
+    g.B = btov(); g.b_rows = (long long)P.o * v;        // rows n = (x, p)
     g.m1_base = 0; g.m1_ext = v; g.m2_ext = v;
     g.n_base = r.orb0 * v; g.n_ext = (long long)r.len * v;
-    g.c_off = (long long)slot0 * (long long)P.slab_elems;
     g.sM1 = P.Kp; g.sM2 = 1; g.sN1 = 0; g.sN2 = (long long)v * P.Kp; g.n2_ext = INT_MAX;
-    g.C = c.slabs();
-    // DF tasks are all "single term, a_idx = b_idx = 0" and differ only in c_off; slot reserved in build_schedule
-    BQC_TRY(run_df_gemm(c, g, form_task_slot[(size_t)block * P.nsets * P.na + (size_t)set * P.na + r.pos0], s));
-    BQC_TRY(launch_slab_holes(c.in.t2, c.slabs(), P.o, v, P.Kp, r.orb0, r.len, slot0, s));
+    g.C = slabs() + (size_t)slot0 * P.slab_elems;
+    BQC_TRY(run_df_gemm(g, s));
+    BQC_TRY(launch_slab_holes(in.t2, slabs(), P.o, v, P.Kp, r.orb0, r.len, slot0, P.dual, s));
   }
   return BQC_OK;
 }
 
-int Pipeline::build_schedule() {
-  Plan& P = c.P;
-  const int na = P.na, v = P.v;
-  // ---- DF task slots first: (z-run, y-run) pairs for B~/J, then one per (block, set, run) for slabs
-  const std::vector<Run> runs = runs_of(P.act, 0, na);
-  for (const Run& rz : runs)
-    for (const Run& ry : runs) {
-      push_task(c, single_term_task(((long long)rz.pos0 * na + ry.pos0) * v * P.Kp + v));
-      push_task(c, single_term_task(((long long)rz.pos0 * na + ry.pos0) * v * v));
-    }
-  form_task_slot.assign((size_t)P.nblk * P.nsets * na, (size_t)-1);
-  for (int b = 0; b < P.nblk; ++b)
-    for (int set = 0; set < P.nsets; ++set)
-      for (const Run& r : runs_of(P.act, block_begin(b), block_end(b))) {
-        const int slot0 = set * P.Bo + (r.pos0 - block_begin(b));
-        form_task_slot[(size_t)b * P.nsets * na + (size_t)set * na + r.pos0] =
-            push_task(c, single_term_task((long long)slot0 * (long long)P.slab_elems));
-      }
-
-  // ---- block triples I <= J <= K with the slot-set protocol: I -> set 0, J -> set 1, K -> sets 2/3
-  int set_block[4] = {-1, -1, -1, -1};
-  int kflip = 0;
-  auto acquire = [&](int set, int block) {
-    if (set_block[set] == block) return;
-    Action a;
-    memset(&a, 0, sizeof(a));
-    a.kind = Action::FORM; a.set = set; a.block = block;
-    actions.push_back(a);
-    set_block[set] = block;
-  };
-  auto slot_of = [&](int pos, int set, int block) { return set * P.Bo + (pos - block_begin(block)); };
-
-  long long block_triple = -1;
-  std::vector<int> bt_owner;
-  if (P.shard_blocks) bt_owner = deal_block_triples(na, P.Bo, P.shard_count);
-  for (int I = 0; I < P.nblk; ++I) {
-    for (int Jb = I; Jb < P.nblk; ++Jb) {
-      const int sJ = (Jb == I) ? 0 : 1;
-      for (int K = Jb; K < P.nblk; ++K) {
-        ++block_triple;
-        // BQC_T_FLAG_SHARD_BLOCKS: whole block triples are dealt to the shards, so a shard forms only the
-        // slabs of its own block triples; otherwise every shard owns some triplets of every block triple
-        if (P.shard_blocks && bt_owner[(size_t)block_triple] != P.shard_rank) continue;
-        int sK = sJ;
-        if (K != Jb) sK = (set_block[2] == K) ? 2 : (set_block[3] == K ? 3 : 2 + (kflip++ & 1));
-        // triplets of this block triple owned by this shard
-        std::vector<TripletRec> list;
-        std::vector<int> slots;   // 3 per triplet
-        for (int pi = block_begin(I); pi < block_end(I); ++pi)
-          for (int pj = std::max(pi, block_begin(Jb)); pj < block_end(Jb); ++pj)
-            for (int pk = std::max(pj, block_begin(K)); pk < block_end(K); ++pk) {
-              if (pi == pj && pj == pk) continue;   // g(i,i,i) = 0 exactly
-              TripletRec t;
-              t.i = P.act[pi]; t.j = P.act[pj]; t.k = P.act[pk];
-              t.pi = pi; t.pj = pj; t.pk = pk;
-              t.index = (long long)triplet_index(P.o, t.i, t.j, t.k);
-              if (!P.shard_blocks && (int)(t.index % P.shard_count) != P.shard_rank) continue;
-              list.push_back(t);
-              slots.push_back(slot_of(pi, 0, I));
-              slots.push_back(slot_of(pj, sJ, Jb));
-              slots.push_back(slot_of(pk, sK, K));
-            }
-        if (list.empty()) continue;
-        // slabs are formed only for block triples that have work (the acquire calls are idempotent)
-        acquire(0, I);
-        if (Jb != I) acquire(1, Jb);
-        if (K != Jb) acquire(sK, K);
-        for (size_t b0 = 0; b0 < list.size(); b0 += P.nbatch) {
-          const size_t nb = std::min(list.size() - b0, (size_t)P.nbatch);
-          Action a;
-          memset(&a, 0, sizeof(a));
-          a.kind = Action::COMPUTE;
-          a.trip0 = c.trips.size(); a.ntrip = nb; a.task0 = c.tasks.size();
-          a.sets_used[0] = 0; a.sets_used[1] = sJ; a.sets_used[2] = sK;
-          for (size_t n = 0; n < nb; ++n) {
-            const TripletRec& t = list[b0 + n];
-            const int si = slots[3 * (b0 + n)], sj = slots[3 * (b0 + n) + 1], sk = slots[3 * (b0 + n) + 2];
-            c.trips.push_back(t);
-            auto pair = [&](int pz, int py) { return pz * na + py; };
-            // F(x,y,z): term0 = (I~_x, canonical rows, B~_zy), term1 = (I~_y, transposed rows, B~_zx)
-            auto f_task = [&](int sx, int sy, int px, int py, int pz, int cls) {
-              GemmTask g;
-              memset(&g, 0, sizeof(g));
-              g.nterms = 2;
-              g.term[0].a_idx = sx; g.term[0].a_transposed = 0; g.term[0].b_idx = pair(pz, py);
-              g.term[1].a_idx = sy; g.term[1].a_transposed = 1; g.term[1].b_idx = pair(pz, px);
-              g.c_off = (long long)((n * 3 + cls) * P.fsz);
-              push_task(c, g);
-            };
-            f_task(si, sj, t.pi, t.pj, t.pk, 0);   // F(i,j,k)
-            f_task(si, sk, t.pi, t.pk, t.pj, 1);   // F(i,k,j)
-            f_task(sj, sk, t.pj, t.pk, t.pi, 2);   // F(j,k,i)
-          }
-          actions.push_back(a);
-        }
+// B~ (both halves) and, if asked, J of the pair block (set, block) x (set2, block2)   (row a1).
+int Engine::exec_pair(const Action& a, cudaStream_t s) {
+  const int o = P.o, v = P.v, ns = P.nslots;
+  for (const Run& ry : runs_of(P.act, block_begin(a.block2), block_end(a.block2))) {
+    // K-major panel of the outer-outer DF block: rows ((y - y0) o + l)[Q] = B_outer[Q][y][l]
+    if (a.need_panel || P.nruns > 1)
+      BQC_TRY(launch_transpose_pad(B_outer(), (long long)o * o, (long long)ry.orb0 * o, (long long)ry.len * o,
+                                   panel(), P.X, P.Xp, 0, 0, s));
+    const int sy0 = slot_of(ry.pos0, a.set2, a.block2);
+    for (const Run& rz : runs_of(P.act, block_begin(a.block), block_end(a.block))) {
+      const int sz0 = slot_of(rz.pos0, a.set, a.block);
+      const size_t pair0 = (size_t)sz0 * ns + sy0;
+      BQC_TRY(launch_btilde_t2(in.t2, btil(), o, v, P.Kp, ns, rz.orb0, rz.len, ry.orb0, ry.len, sz0, sy0, P.dual, s));
+      DfGemm g;   // hole columns: B~_zy[r, v + l] = (z r|y l)
+      g.A = btov(); g.a_d1 = v; g.a_d2 = o;
+      g.B = panel(); g.b_rows = (long long)ry.len * o;
+      g.m1_base = rz.orb0; g.m1_ext = rz.len; g.m2_ext = v;
+      g.n_base = 0; g.n_ext = (long long)ry.len * o;
+      g.sM1 = (long long)ns * v * P.Kp; g.sM2 = P.Kp; g.sN1 = (long long)v * P.Kp; g.sN2 = 1; g.n2_ext = o;
+      g.C = btil() + pair0 * v * P.Kp + v;
+      BQC_TRY(run_df_gemm(g, s));
+      if (a.need_j) {
+        DfGemm j;   // J_zy[u, w] = (z u|y w)
+        j.A = btov(); j.a_d1 = v; j.a_d2 = o;
+        j.B = btov(); j.b_rows = (long long)o * v;
+        j.m1_base = rz.orb0; j.m1_ext = rz.len; j.m2_ext = v;
+        j.n_base = ry.orb0 * v; j.n_ext = (long long)ry.len * v;
+        j.sM1 = (long long)ns * v * v; j.sM2 = v; j.sN1 = (long long)v * v; j.sN2 = 1; j.n2_ext = v;
+        j.C = J() + pair0 * v * v;
+        BQC_TRY(run_df_gemm(j, s));
       }
     }
   }
   return BQC_OK;
 }
 
-int Pipeline::compute(const Action& a) {
-  const Plan& P = c.P;
-  cudaStream_t s = c.s_main;
-  const int v = P.v;
+int Engine::exec_compute(int chunk, size_t trip0, size_t ntrip, cudaStream_t s) {
   GemmParams prm;
   memset(&prm, 0, sizeof(prm));
-  prm.ntasks = (int)(3 * a.ntrip);
-  prm.tasks = c.tasks_dev() + a.task0;
-  prm.C = c.F();
-  if (P.profile) BQC_TRY(c.prof_mark(c.prof_main, s));
-  BQC_TRY(launch_f_gemm(c, prm, s));
-  if (P.profile) BQC_TRY(c.prof_mark(c.prof_main, s));
+  prm.ntasks = (int)(3 * ntrip);
+  prm.tasks = tasks_dev(chunk) + 3 * trip0;
+  prm.C = F();
+  if (P.profile) BQC_TRY(prof_mark(prof_main, s));
+  BQC_TRY(launch_f_gemm(prm, s));
+  if (P.profile) BQC_TRY(prof_mark(prof_main, s));
 
   EnergyArgs e;
-  e.F = c.F(); e.trips = c.trips_dev() + a.trip0; e.orbits = c.orbits_dev();
-  e.J = c.J(); e.t1 = c.in.t1; e.eps_occ = c.in.eps_occ; e.eps_vir = c.in.eps_vir;
-  e.partial = c.partial();
-  e.t2 = c.in.t2; e.f_ov = c.in.f_ov; e.o = P.o;
-  e.ntrip = (int)a.ntrip; e.norbits = P.norbits; e.nbv = P.nbv; e.v = v; e.nw = P.na; e.use_t1 = P.use_t1;
+  e.F = F(); e.trips = trips_dev(chunk) + trip0; e.orbits = orbits_dev();
+  e.J = J(); e.t1 = t1p(); e.eps_occ = eps_o(); e.eps_vir = eps_v();
+  e.partial = partial();
+  e.t2 = in.t2; e.f_ov = fp(); e.o = P.o; e.dual = P.dual ? 1 : 0;
+  e.ntrip = (int)ntrip; e.norbits = P.norbits; e.nbv = P.nbv; e.v = P.v; e.nw = P.nslots; e.use_t1 = P.use_t1;
   BQC_TRY(launch_energy(e, s));
-  BQC_TRY(launch_reduce_triplets(c.partial(), c.trips_dev() + a.trip0, (int)a.ntrip, P.norbits, c.etrip(), s));
-  if (P.profile) BQC_TRY(c.prof_mark(c.prof_main, s));
+  BQC_TRY(launch_reduce_triplets(partial(), trips_dev(chunk) + trip0, (int)ntrip, P.norbits, etrip(), s));
+  if (P.profile) BQC_TRY(prof_mark(prof_main, s));
   return BQC_OK;
 }
 
-int Pipeline::execute() {
+// One block triple: its triplet records and F tasks are written into the next pinned chunk, uploaded on the
+// main stream (stream order protects the device chunk: its previous user, two block triples ago, ran earlier
+// on the same stream), and evaluated `nbatch` triplets per W-builder launch.
+int Engine::exec_triple(const Action& a, cudaStream_t s) {
+  const int b = chunk_next;
+  chunk_next ^= 1;
+  if (ev_up_valid[b]) BQC_CUDA_OK(cudaEventSynchronize(ev_up[b]));   // the upload that last read this pinned half
+  const size_t n = list_triple(a, trips_host(b), tasks_host(b));
+  BQC_CUDA_OK(cudaMemcpyAsync(trips_dev(b), trips_host(b), n * sizeof(TripletRec), cudaMemcpyHostToDevice, s));
+  BQC_CUDA_OK(cudaMemcpyAsync(tasks_dev(b), tasks_host(b), 3 * n * sizeof(GemmTask), cudaMemcpyHostToDevice, s));
+  BQC_CUDA_OK(cudaEventRecord(ev_up[b], s));
+  ev_up_valid[b] = true;
+  for (size_t t0 = 0; t0 < n; t0 += P.nbatch)
+    BQC_TRY(exec_compute(b, t0, std::min(n - t0, (size_t)P.nbatch), s));
+  return BQC_OK;
+}
+
+int Engine::execute() {
   for (const Action& a : actions) {
     if (a.kind == Action::FORM) {
       // the former stream may overwrite a slot set only after the main stream's last use of it
-      if (c.ev_free_valid[a.set]) BQC_CUDA_OK(cudaStreamWaitEvent(c.s_form, c.ev_free[a.set], 0));
-      if (c.P.profile) BQC_TRY(c.prof_mark(c.prof_form, c.s_form));
-      BQC_TRY(form_block(a.set, a.block, c.s_form));
-      if (c.P.profile) BQC_TRY(c.prof_mark(c.prof_form, c.s_form));
-      BQC_CUDA_OK(cudaEventRecord(c.ev_formed[a.set], c.s_form));
-      BQC_CUDA_OK(cudaStreamWaitEvent(c.s_main, c.ev_formed[a.set], 0));
+      if (ev_free_valid[a.set]) BQC_CUDA_OK(cudaStreamWaitEvent(s_form, ev_free[a.set], 0));
+      if (P.profile) BQC_TRY(prof_mark(prof_form, s_form));
+      BQC_TRY(exec_form(a.set, a.block, s_form));
+      if (P.profile) BQC_TRY(prof_mark(prof_form, s_form));
+      BQC_CUDA_OK(cudaEventRecord(ev_formed[a.set], s_form));
+      BQC_CUDA_OK(cudaStreamWaitEvent(s_main, ev_formed[a.set], 0));
+    } else if (a.kind == Action::PAIR) {
+      // pair blocks are written and read on the main stream only: stream order is the only ordering needed
+      if (P.profile) BQC_TRY(prof_mark(prof_form, s_main));
+      BQC_TRY(exec_pair(a, s_main));
+      if (P.profile) BQC_TRY(prof_mark(prof_form, s_main));
     } else {
-      BQC_TRY(compute(a));
+      BQC_TRY(exec_triple(a, s_main));
+      const int used[3] = {0, a.sJ, a.sK};
       for (int n = 0; n < 3; ++n) {
-        const int set = a.sets_used[n];
-        BQC_CUDA_OK(cudaEventRecord(c.ev_free[set], c.s_main));
-        c.ev_free_valid[set] = true;
+        BQC_CUDA_OK(cudaEventRecord(ev_free[used[n]], s_main));
+        ev_free_valid[used[n]] = true;
       }
     }
   }
   // join the former stream back into the caller's stream
-  BQC_CUDA_OK(cudaEventRecord(c.ev_join, c.s_form));
-  BQC_CUDA_OK(cudaStreamWaitEvent(c.s_main, c.ev_join, 0));
+  BQC_CUDA_OK(cudaEventRecord(ev_join, s_form));
+  BQC_CUDA_OK(cudaStreamWaitEvent(s_main, ev_join, 0));
   return BQC_OK;
 }
 
-// ------------------------------------------------------------------ common front end
+// ------------------------------------------------------------------ one evaluation
 int validate_inputs(int o, int v, int X, const Inputs& in) {
   BQC_TRY(check_sizes(o, v, X));
   BQC_TRY(check_device());
@@ -768,189 +672,157 @@ int validate_inputs(int o, int v, int X, const Inputs& in) {
   BQC_TRY(check_device_ptr(in.B_oo, "B_oo"));
   BQC_TRY(check_device_ptr(in.B_ov, "B_ov"));
   BQC_TRY(check_device_ptr(in.B_vv, "B_vv"));
+  if (in.f_ov) BQC_TRY(check_device_ptr(in.f_ov, "opts->f_ov"));
   return BQC_OK;
 }
 
-int check_denominators(int o, int v, const Inputs& in, cudaStream_t s) {
-  std::vector<double> eo(o), ev(v);
-  BQC_CUDA_OK(cudaMemcpyAsync(eo.data(), in.eps_occ, (size_t)o * 8, cudaMemcpyDeviceToHost, s));
-  BQC_CUDA_OK(cudaMemcpyAsync(ev.data(), in.eps_vir, (size_t)v * 8, cudaMemcpyDeviceToHost, s));
-  BQC_CUDA_OK(cudaStreamSynchronize(s));
-  const double emax = *std::max_element(eo.begin(), eo.end());
-  const double vmin = *std::min_element(ev.begin(), ev.end());
-  if (!(3.0 * emax - 3.0 * vmin < 0.0)) {
-    set_error(BQC_ERR_DENOMINATOR, "3*max(eps_occ)=%g - 3*min(eps_vir)=%g >= 0: denominators may vanish",
-              3.0 * emax, 3.0 * vmin);
-    return BQC_ERR_DENOMINATOR;
+int denominator_error(double emax, double vmin) {
+  set_error(BQC_ERR_DENOMINATOR, "3*max(eps_occ)=%g - 3*min(eps_vir)=%g >= 0: denominators may vanish",
+            3.0 * emax, 3.0 * vmin);
+  return BQC_ERR_DENOMINATOR;
+}
+
+int Engine::run(const Inputs& inputs, double* e_total_host, double* e_triplet_dev, cudaStream_t stream) {
+  in = inputs;
+  s_main = stream;
+  const bool prof = P.profile != 0;
+  const long long launches0 = g_launches;
+  ev_used = 0;
+  prof_main.clear();
+  prof_form.clear();
+  // Reading G10: refuse inputs whose denominators can vanish.  A long run checks before it starts (one
+  // blocking 8(o+v)-byte read-back); a short one lets a kernel evaluate the bound on the stream and reads the
+  // verdict together with the result, so that the call has a single host synchronisation.
+  const bool check_first = ncompute > 64;
+  if (check_first) {
+    std::vector<double> eo(nocc), ev(nvir);
+    BQC_CUDA_OK(cudaMemcpyAsync(eo.data(), in.eps_occ, (size_t)nocc * 8, cudaMemcpyDeviceToHost, stream));
+    BQC_CUDA_OK(cudaMemcpyAsync(ev.data(), in.eps_vir, (size_t)nvir * 8, cudaMemcpyDeviceToHost, stream));
+    BQC_CUDA_OK(cudaStreamSynchronize(stream));
+    const double emax = *std::max_element(eo.begin(), eo.end());
+    const double vmin = *std::min_element(ev.begin(), ev.end());
+    if (!(3.0 * emax - 3.0 * vmin < 0.0)) return denominator_error(emax, vmin);
+  }
+  if (prof) {
+    if (!prof_begin) {
+      BQC_CUDA_OK(cudaEventCreate(&prof_begin));
+      BQC_CUDA_OK(cudaEventCreate(&prof_prepared));
+      BQC_CUDA_OK(cudaEventCreate(&prof_end));
+    }
+    BQC_CUDA_OK(cudaEventRecord(prof_begin, stream));
+  }
+  // esum: [0] E, [1] denominator verdict (0 ok), [2] max eps_occ, [3] min eps_vir
+  BQC_CUDA_OK(cudaMemsetAsync(esum(), 0, 32, stream));
+  if (!check_first) BQC_TRY(launch_denominator_check(in.eps_occ, nocc, in.eps_vir, nvir, esum() + 1, stream));
+  BQC_TRY(prepare(stream));
+  if (prof) BQC_CUDA_OK(cudaEventRecord(prof_prepared, stream));
+  BQC_TRY(execute());
+  BQC_TRY(launch_final_sum(etrip(), (long long)num_triplets(P.o), esum(), stream));
+  if (prof) BQC_CUDA_OK(cudaEventRecord(prof_end, stream));
+  if (e_triplet_dev)
+    BQC_CUDA_OK(cudaMemcpyAsync(e_triplet_dev, etrip(), num_triplets(P.o) * 8, cudaMemcpyDeviceToDevice, stream));
+  double res[4] = {0, 0, 0, 0};
+  BQC_CUDA_OK(cudaMemcpyAsync(res, esum(), 32, cudaMemcpyDeviceToHost, stream));
+  BQC_CUDA_OK(cudaStreamSynchronize(stream));   // joins s_form too (ev_join)
+  g_profile[8] = (double)(g_launches - launches0);
+  if (res[1] != 0.0) return denominator_error(res[2], res[3]);
+  *e_total_host = res[0];
+  if (prof) {
+    double gemm_ms = 0, en_ms = 0, form_ms = 0;
+    float ms = 0.f;
+    for (size_t n = 0; n + 2 < prof_main.size() + 1; n += 3) {
+      BQC_CUDA_OK(cudaEventElapsedTime(&ms, prof_main[n], prof_main[n + 1]));
+      gemm_ms += ms;
+      BQC_CUDA_OK(cudaEventElapsedTime(&ms, prof_main[n + 1], prof_main[n + 2]));
+      en_ms += ms;
+    }
+    for (size_t n = 0; n + 1 < prof_form.size(); n += 2) {
+      BQC_CUDA_OK(cudaEventElapsedTime(&ms, prof_form[n], prof_form[n + 1]));
+      form_ms += ms;
+    }
+    size_t nform = 0;
+    for (const Action& a : actions) nform += (a.kind == Action::FORM);
+    g_profile[0] = gemm_ms;
+    g_profile[1] = (double)(prof_main.size() / 3);
+    g_profile[2] = en_ms;
+    g_profile[3] = (double)(prof_main.size() / 3);
+    g_profile[4] = form_ms;
+    g_profile[5] = (double)nform;
+    BQC_CUDA_OK(cudaEventElapsedTime(&ms, prof_begin, prof_prepared));
+    g_profile[6] = ms;
+    BQC_CUDA_OK(cudaEventElapsedTime(&ms, prof_begin, prof_end));
+    g_profile[7] = ms;
   }
   return BQC_OK;
 }
 
-int t_energy_impl(int o, int v, int X, const Inputs& in, const bqc_t_opts* opts, void* workspace,
+// ------------------------------------------------------------------ engine reuse
+// The last engine of this thread is kept and reused when the next call has the same sizes, options,
+// workspace and device: its streams, events, tensor maps and schedule are then not rebuilt.  An engine that
+// owns its workspace is kept only while that workspace is small (kKeepBytes); bqc_release_cached() drops it.
+constexpr size_t kKeepBytes = (size_t)2 << 30;
+thread_local std::unique_ptr<Engine> g_engine;
+
+bool same_opts(const bqc_t_opts& a, const bqc_t_opts* b) {
+  bqc_t_opts z;
+  memset(&z, 0, sizeof(z));
+  if (b) z = *b;
+  return a.occ_block == z.occ_block && a.occ_lo == z.occ_lo && a.occ_hi == z.occ_hi &&
+         a.shard_rank == z.shard_rank && a.shard_count == z.shard_count && a.max_batch == z.max_batch &&
+         a.flags == z.flags && a.workspace_gib == z.workspace_gib && (a.f_ov != nullptr) == (z.f_ov != nullptr);
+}
+
+int engine_for(int nocc, int nvir, int naux, const bqc_t_opts* opts, void* workspace, size_t workspace_bytes,
+               Engine** out) {
+  int dev = -1;
+  BQC_CUDA_OK(cudaGetDevice(&dev));
+  Engine* e = g_engine.get();
+  if (e && e->nocc == nocc && e->nvir == nvir && e->naux == naux && e->device == dev && e->key_ws == workspace &&
+      e->key_ws_bytes == workspace_bytes && same_opts(e->key_opts, opts)) {
+    *out = e;
+    return BQC_OK;
+  }
+  g_engine.reset();   // frees the old workspace before the new one is allocated
+  std::unique_ptr<Engine> fresh(new Engine());
+  BQC_TRY(fresh->init(nocc, nvir, naux, opts, workspace, workspace_bytes, nullptr));
+  g_engine = std::move(fresh);
+  *out = g_engine.get();
+  return BQC_OK;
+}
+
+int t_energy_impl(int nocc, int nvir, int naux, const Inputs& in, const bqc_t_opts* opts, void* workspace,
                   size_t workspace_bytes, double* e_total_host, double* e_triplet_dev, cudaStream_t stream) {
   clear_error();
   if (!e_total_host) {
     set_error(BQC_ERR_NULL_POINTER, "e_total_host is NULL");
     return BQC_ERR_NULL_POINTER;
   }
-  BQC_TRY(validate_inputs(o, v, X, in));
-  if (in.f_ov) BQC_TRY(check_device_ptr(in.f_ov, "opts->f_ov"));
+  BQC_TRY(validate_inputs(nocc, nvir, naux, in));
   if (e_triplet_dev) BQC_TRY(check_device_ptr(e_triplet_dev, "e_triplet_dev"));
+  const bool dual = opts && (opts->flags & BQC_T_FLAG_ABC_DRIVEN);
+  const int o = dual ? nvir : nocc;   // extent of the outer index
   int lo, hi;
   BQC_TRY(resolve_window(o, opts, &lo, &hi));
-  BQC_TRY(check_denominators(o, v, in, stream));
-  if (hi - lo < 2) {   // a single occupied orbital: two electrons, no triples
-    *e_total_host = 0.0;
+  if (hi - lo < 2) {
+    // a single outer orbital: only the diagonal triplet, which contributes exactly 0;
+    // nocc = 1 is two electrons, no triples.  The denominator precondition (G10) is still checked.
+    std::vector<double> eo(nocc), ev(nvir);
+    BQC_CUDA_OK(cudaMemcpyAsync(eo.data(), in.eps_occ, (size_t)nocc * 8, cudaMemcpyDeviceToHost, stream));
+    BQC_CUDA_OK(cudaMemcpyAsync(ev.data(), in.eps_vir, (size_t)nvir * 8, cudaMemcpyDeviceToHost, stream));
     if (e_triplet_dev) BQC_CUDA_OK(cudaMemsetAsync(e_triplet_dev, 0, num_triplets(o) * 8, stream));
     BQC_CUDA_OK(cudaStreamSynchronize(stream));
+    const double emax = *std::max_element(eo.begin(), eo.end());
+    const double vmin = *std::min_element(ev.begin(), ev.end());
+    if (!(3.0 * emax - 3.0 * vmin < 0.0)) return denominator_error(emax, vmin);
+    *e_total_host = 0.0;
     return BQC_OK;
   }
-  std::vector<int> act;
-  for (int x = lo; x < hi; ++x) act.push_back(x);
-
-  Pipeline p;
-  BQC_TRY(p.setup(o, v, X, in, act, opts, workspace, workspace_bytes, stream));
-  Ctx& c = p.c;
-  const bool prof = c.P.profile != 0;
-  const long long launches0 = g_launches;
-  if (prof) {
-    BQC_CUDA_OK(cudaEventCreate(&c.prof_begin));
-    BQC_CUDA_OK(cudaEventCreate(&c.prof_prepared));
-    BQC_CUDA_OK(cudaEventCreate(&c.prof_end));
-    BQC_CUDA_OK(cudaEventRecord(c.prof_begin, stream));
-  }
-  BQC_TRY(p.build_schedule());
-  BQC_TRY(p.prepare());
-  if (prof) BQC_CUDA_OK(cudaEventRecord(c.prof_prepared, stream));
-  BQC_TRY(p.execute());
-  BQC_TRY(launch_final_sum(c.etrip(), (long long)num_triplets(o), c.esum(), stream));
-  if (prof) BQC_CUDA_OK(cudaEventRecord(c.prof_end, stream));
-  if (e_triplet_dev)
-    BQC_CUDA_OK(cudaMemcpyAsync(e_triplet_dev, c.etrip(), num_triplets(o) * 8, cudaMemcpyDeviceToDevice, stream));
-  BQC_CUDA_OK(cudaMemcpyAsync(e_total_host, c.esum(), 8, cudaMemcpyDeviceToHost, stream));
-  BQC_CUDA_OK(cudaStreamSynchronize(stream));
-  BQC_CUDA_OK(cudaStreamSynchronize(c.s_form));
-  g_profile[8] = (double)(g_launches - launches0);
-  if (prof) {
-    double gemm_ms = 0, en_ms = 0, form_ms = 0;
-    float ms = 0.f;
-    for (size_t n = 0; n + 2 < c.prof_main.size() + 1; n += 3) {
-      BQC_CUDA_OK(cudaEventElapsedTime(&ms, c.prof_main[n], c.prof_main[n + 1]));
-      gemm_ms += ms;
-      BQC_CUDA_OK(cudaEventElapsedTime(&ms, c.prof_main[n + 1], c.prof_main[n + 2]));
-      en_ms += ms;
-    }
-    for (size_t n = 0; n + 1 < c.prof_form.size(); n += 2) {
-      BQC_CUDA_OK(cudaEventElapsedTime(&ms, c.prof_form[n], c.prof_form[n + 1]));
-      form_ms += ms;
-    }
-    g_profile[0] = gemm_ms;
-    g_profile[1] = (double)(c.prof_main.size() / 3);
-    g_profile[2] = en_ms;
-    g_profile[3] = (double)(c.prof_main.size() / 3);
-    g_profile[4] = form_ms;
-    g_profile[5] = (double)(c.prof_form.size() / 2);
-    BQC_CUDA_OK(cudaEventElapsedTime(&ms, c.prof_begin, c.prof_prepared));
-    g_profile[6] = ms;
-    BQC_CUDA_OK(cudaEventElapsedTime(&ms, c.prof_begin, c.prof_end));
-    g_profile[7] = ms;
-  }
-  return BQC_OK;
-}
-
-// ------------------------------------------------------------------ abc-driven schedule
-// The paper's loop is over virtual triples a,b,c with o^3 tensors per iteration.  The
-// contraction of Eq. (2) is invariant under exchanging the roles of occupied and virtual orbitals
-// (DESIGN.md §12): with
-//     o' = v, v' = o, eps_occ' = -eps_vir, eps_vir' = -eps_occ, t1'[a,i] = t1[i,a],
-//     t2'[a,b,i,j] = -t2[i,j,a,b], B_oo' = B_vv, B_vv' = B_oo, B_ov'[Q,a,i] = B_ov[Q,i,a], f'[a,i] = -f[i,a]
-// the dual problem's triplet (a <= b <= c) carries W_abc[i,j,k] for all i,j,k, its "slabs" are the o^2 (v+o)
-// pieces (zr|yl), t2[z,y,r,:] of one virtual r and its per-triplet value is the abc-driven contribution
-// (2 - d_ab - d_bc) sum_ijk R V / D.  So the abc-driven schedule is the same pipeline on the dual arrays,
-// which are built here on the device (one pass over t2 and B_ov).
-struct DualLayout {
-  size_t off_eo = 0, off_ev = 0, off_t1 = 0, off_f = 0, off_bov = 0, off_t2 = 0, total = 0;
-};
-
-DualLayout dual_layout(int o, int v, int X, bool fock) {
-  DualLayout L;
-  size_t off = 0;
-  auto take = [&](size_t bytes) { size_t r = off; off = round_up(off + bytes, 1024); return r; };
-  L.off_eo = take((size_t)v * 8);
-  L.off_ev = take((size_t)o * 8);
-  L.off_t1 = take((size_t)o * v * 8);
-  L.off_f = take(fock ? (size_t)o * v * 8 : 0);
-  L.off_bov = take((size_t)X * o * v * 8);
-  L.off_t2 = take((size_t)o * o * v * v * 8);
-  L.total = off;
-  return L;
-}
-
-bqc_t_opts dual_opts(const bqc_t_opts* opts) {
-  bqc_t_opts d;
-  memset(&d, 0, sizeof(d));
-  if (opts) d = *opts;
-  d.flags &= ~BQC_T_FLAG_ABC_DRIVEN;
-  d.f_ov = nullptr;
-  return d;
-}
-
-int t_energy_abc(int o, int v, int X, const Inputs& in, const bqc_t_opts* opts, void* workspace,
-                 size_t workspace_bytes, double* e_total_host, double* e_triplet_dev, cudaStream_t stream) {
-  clear_error();
-  if (!e_total_host) {
-    set_error(BQC_ERR_NULL_POINTER, "e_total_host is NULL");
-    return BQC_ERR_NULL_POINTER;
-  }
-  BQC_TRY(validate_inputs(o, v, X, in));
-  if (in.f_ov) BQC_TRY(check_device_ptr(in.f_ov, "opts->f_ov"));
-  bqc_t_opts dopts = dual_opts(opts);
-  int lo, hi;
-  BQC_TRY(resolve_window(v, &dopts, &lo, &hi));
-  Plan P;
-  {
-    std::vector<int> act(hi - lo);
-    for (int x = lo; x < hi; ++x) act[x - lo] = x;
-    BQC_TRY(make_plan(P, v, o, X, act, &dopts));
-  }
-  const DualLayout L = dual_layout(o, v, X, in.f_ov != nullptr);
-  const size_t need = L.total + P.total;
-  uint8_t* ws = static_cast<uint8_t*>(workspace);
-  bool own = false;
-  if (ws) {
-    if (workspace_bytes < need || (reinterpret_cast<uintptr_t>(ws) & 255)) {
-      set_error(BQC_ERR_WORKSPACE, "workspace of %zu bytes (need %zu, 256-byte aligned)", workspace_bytes, need);
-      return BQC_ERR_WORKSPACE;
-    }
-  } else {
-    void* p = nullptr;
-    cudaError_t e = cudaMalloc(&p, need);
-    if (e != cudaSuccess) {
-      cudaGetLastError();
-      set_error(BQC_ERR_WORKSPACE, "cudaMalloc of %zu workspace bytes failed: %s", need, cudaGetErrorString(e));
-      return BQC_ERR_WORKSPACE;
-    }
-    ws = static_cast<uint8_t*>(p);
-    own = true;
-  }
-  auto D = [&](size_t off) { return reinterpret_cast<double*>(ws + off); };
-  const long long launches0 = g_launches;
-  int rc = launch_transpose_scale(in.eps_vir, D(L.off_eo), 1, 1, v, -1.0, stream);
-  if (rc == BQC_OK) rc = launch_transpose_scale(in.eps_occ, D(L.off_ev), 1, 1, o, -1.0, stream);
-  if (rc == BQC_OK) rc = launch_transpose_scale(in.t1, D(L.off_t1), 1, o, v, 1.0, stream);
-  if (rc == BQC_OK && in.f_ov) rc = launch_transpose_scale(in.f_ov, D(L.off_f), 1, o, v, -1.0, stream);
-  if (rc == BQC_OK) rc = launch_transpose_scale(in.B_ov, D(L.off_bov), X, o, v, 1.0, stream);
-  if (rc == BQC_OK)
-    rc = launch_transpose_scale(in.t2, D(L.off_t2), 1, (long long)o * o, (long long)v * v, -1.0, stream);
-  if (rc == BQC_OK) {
-    Inputs din = {D(L.off_eo), D(L.off_ev), D(L.off_t1), D(L.off_t2), in.B_vv, D(L.off_bov), in.B_oo,
-                  in.f_ov ? D(L.off_f) : nullptr};
-    rc = t_energy_impl(v, o, X, din, &dopts, ws + L.total, P.total, e_total_host, e_triplet_dev, stream);
-    g_profile[8] = (double)(g_launches - launches0);
-  }
-  if (own) {
+  Engine* e = nullptr;
+  BQC_TRY(engine_for(nocc, nvir, naux, opts, workspace, workspace_bytes, &e));
+  const int rc = e->run(in, e_total_host, e_triplet_dev, stream);
+  if (rc != BQC_OK || (e->own_ws && e->P.total > kKeepBytes)) {
     cudaStreamSynchronize(stream);
-    cudaFree(ws);
+    g_engine.reset();
   }
   return rc;
 }
@@ -962,110 +834,6 @@ int t_energy_abc(int o, int v, int X, const Inputs& in, const bqc_t_opts* opts, 
 using namespace bqc;
 
 extern "C" {
-
-size_t bqc_t_num_triplets(int nocc) { return nocc > 0 ? num_triplets(nocc) : 0; }
-
-size_t bqc_t_triplet_index(int nocc, int i, int j, int k) {
-  if (nocc <= 0 || i < 0 || i > j || j > k || k >= nocc) return (size_t)-1;
-  return triplet_index(nocc, i, j, k);
-}
-
-int bqc_t_triplet_owner(int nocc, int shard_count, int i, int j, int k) {
-  const size_t idx = bqc_t_triplet_index(nocc, i, j, k);
-  if (idx == (size_t)-1 || shard_count <= 0) return -1;
-  return (int)(idx % (size_t)shard_count);
-}
-
-int bqc_t_triplet_owner_ex(int nocc, int nvir, int naux, const bqc_t_opts* opts, int i, int j, int k) {
-  clear_error();
-  if (check_sizes(nocc, nvir, naux) != BQC_OK) return -1;
-  if (opts && (opts->flags & BQC_T_FLAG_ABC_DRIVEN)) {   // (i,j,k) are virtual indices a<=b<=c
-    const bqc_t_opts d = dual_opts(opts);
-    return bqc_t_triplet_owner_ex(nvir, nocc, naux, &d, i, j, k);
-  }
-  int lo, hi;
-  if (resolve_window(nocc, opts, &lo, &hi) != BQC_OK) return -1;
-  if (i < lo || i > j || j > k || k >= hi) return -1;
-  const int sc = (opts && opts->shard_count > 0) ? opts->shard_count : 1;
-  if (!(opts && (opts->flags & BQC_T_FLAG_SHARD_BLOCKS)))
-    return (int)(triplet_index(nocc, i, j, k) % (size_t)sc);
-  Plan P;
-  std::vector<int> act(hi - lo);
-  for (int x = lo; x < hi; ++x) act[x - lo] = x;
-  bqc_t_opts o2 = *opts;
-  o2.shard_rank = 0;
-  if (make_plan(P, nocc, nvir, naux, act, &o2) != BQC_OK) return -1;
-  // block triples I <= J <= K are numbered in loop order = lexicographic rank among the nblk blocks
-  const size_t bt = triplet_index(P.nblk, (i - lo) / P.Bo, (j - lo) / P.Bo, (k - lo) / P.Bo);
-  return deal_block_triples(P.na, P.Bo, sc)[bt];
-}
-
-double bqc_t_flops(int nocc, int nvir, const bqc_t_opts* opts) {
-  clear_error();
-  if (nocc <= 0 || nvir <= 0) return 0.0;
-  if (opts && (opts->flags & BQC_T_FLAG_ABC_DRIVEN)) {   // virtual triples a<=b<=c, 12 o^3 (v+o) each
-    const bqc_t_opts d = dual_opts(opts);
-    return bqc_t_flops(nvir, nocc, &d);
-  }
-  int lo, hi;
-  if (resolve_window(nocc, opts, &lo, &hi) != BQC_OK) return -1.0;
-  const int sc = (opts && opts->shard_count > 0) ? opts->shard_count : 1;
-  const int sr = opts ? opts->shard_rank : 0;
-  size_t n = 0;
-  if (opts && (opts->flags & BQC_T_FLAG_SHARD_BLOCKS) && sc > 1) {
-    // same block-triple walk as Pipeline::build_schedule (the block size does not depend on naux)
-    Plan P;
-    std::vector<int> act(hi - lo);
-    for (int x = lo; x < hi; ++x) act[x - lo] = x;
-    if (make_plan(P, nocc, nvir, 1, act, opts) != BQC_OK) return -1.0;
-    std::vector<long long> load;
-    deal_block_triples(P.na, P.Bo, sc, &load);
-    n = (size_t)load[sr];
-    const double v = nvir;
-    return (double)n * 12.0 * v * v * v * (v + nocc);
-  }
-  for (int i = lo; i < hi; ++i)
-    for (int j = i; j < hi; ++j)
-      for (int k = j; k < hi; ++k) {
-        if (i == j && j == k) continue;
-        if ((int)(triplet_index(nocc, i, j, k) % (size_t)sc) == sr) ++n;
-      }
-  const double v = nvir;
-  return (double)n * 12.0 * v * v * v * (v + nocc);
-}
-
-int bqc_t_plan_occ_block(int nocc, int nvir, int naux, const bqc_t_opts* opts) {
-  clear_error();
-  if (check_sizes(nocc, nvir, naux) != BQC_OK) return -1;
-  if (opts && (opts->flags & BQC_T_FLAG_ABC_DRIVEN)) {   // block size over the virtual index
-    const bqc_t_opts d = dual_opts(opts);
-    return bqc_t_plan_occ_block(nvir, nocc, naux, &d);
-  }
-  int lo, hi;
-  if (resolve_window(nocc, opts, &lo, &hi) != BQC_OK) return -1;
-  Plan P;
-  std::vector<int> act(hi - lo);
-  for (int x = lo; x < hi; ++x) act[x - lo] = x;
-  if (make_plan(P, nocc, nvir, naux, act, opts) != BQC_OK) return -1;
-  return P.Bo;
-}
-
-size_t bqc_t_workspace_bytes(int nocc, int nvir, int naux, const bqc_t_opts* opts) {
-  clear_error();
-  if (check_sizes(nocc, nvir, naux) != BQC_OK) return 0;
-  if (opts && (opts->flags & BQC_T_FLAG_ABC_DRIVEN)) {   // dual arrays + the dual problem's workspace
-    const bqc_t_opts d = dual_opts(opts);
-    const size_t inner = bqc_t_workspace_bytes(nvir, nocc, naux, &d);
-    return inner ? dual_layout(nocc, nvir, naux, opts->f_ov != nullptr).total + inner : 0;
-  }
-  int lo, hi;
-  if (resolve_window(nocc, opts, &lo, &hi) != BQC_OK) return 0;
-  Plan P;
-  std::vector<int> act(hi - lo);
-  for (int x = lo; x < hi; ++x) act[x - lo] = x;
-  if (make_plan(P, nocc, nvir, naux, act, opts) != BQC_OK) return 0;
-  return P.total;
-}
 
 int bqc_sum_in_order(const double* x, size_t n, double* out_host, void* stream_v) {
   clear_error();
@@ -1111,7 +879,7 @@ int bqc_t_last_profile(double* out, int n) {
 
 int bqc_last_error(void) { return g_err; }
 const char* bqc_error_detail(void) { return g_detail; }
-const char* bqc_version(void) { return "bqc_t 0.1 (sm_100a)"; }
+const char* bqc_version(void) { return "bqc_t 0.2 (sm_100a)"; }
 
 const char* bqc_error_string(int code) {
   switch (code) {
@@ -1129,14 +897,13 @@ const char* bqc_error_string(int code) {
   return "unknown error";
 }
 
+void bqc_release_cached(void) { g_engine.reset(); }
+
 int bqc_t_energy_ex(int nocc, int nvir, int naux, const double* eps_occ, const double* eps_vir,
                     const double* t1, const double* t2, const double* B_oo, const double* B_ov,
                     const double* B_vv, const bqc_t_opts* opts, void* workspace, size_t workspace_bytes,
                     double* e_total_host, double* e_triplet_dev, void* stream) {
   Inputs in = {eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, opts ? opts->f_ov : nullptr};
-  if (opts && (opts->flags & BQC_T_FLAG_ABC_DRIVEN))
-    return t_energy_abc(nocc, nvir, naux, in, opts, workspace, workspace_bytes, e_total_host, e_triplet_dev,
-                        static_cast<cudaStream_t>(stream));
   return t_energy_impl(nocc, nvir, naux, in, opts, workspace, workspace_bytes, e_total_host, e_triplet_dev,
                        static_cast<cudaStream_t>(stream));
 }
@@ -1148,6 +915,60 @@ double bqc_t_energy(int nocc, int nvir, int naux, const double* eps_occ, const d
   const int rc = bqc_t_energy_ex(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, nullptr, nullptr,
                                  0, &e, nullptr, stream);
   return rc == BQC_OK ? e : nan("");
+}
+
+// ---- explicit plan handle: the engine without the thread-local cache --------------------------------------
+int bqc_t_plan_create(int nocc, int nvir, int naux, const bqc_t_opts* opts, void* workspace,
+                      size_t workspace_bytes, bqc_t_plan* plan_out) {
+  clear_error();
+  if (!plan_out) {
+    set_error(BQC_ERR_NULL_POINTER, "plan_out is NULL");
+    return BQC_ERR_NULL_POINTER;
+  }
+  *plan_out = nullptr;
+  BQC_TRY(check_sizes(nocc, nvir, naux));
+  BQC_TRY(check_device());
+  if (workspace) BQC_TRY(check_device_ptr(workspace, "workspace"));
+  std::unique_ptr<Engine> e(new Engine());
+  BQC_TRY(e->init(nocc, nvir, naux, opts, workspace, workspace_bytes, nullptr));
+  *plan_out = reinterpret_cast<bqc_t_plan>(e.release());
+  return BQC_OK;
+}
+
+int bqc_t_plan_execute(bqc_t_plan plan, const double* eps_occ, const double* eps_vir, const double* t1,
+                       const double* t2, const double* B_oo, const double* B_ov, const double* B_vv,
+                       const double* f_ov, double* e_total_host, double* e_triplet_dev, void* stream) {
+  clear_error();
+  Engine* e = reinterpret_cast<Engine*>(plan);
+  if (!e || !e_total_host) {
+    set_error(BQC_ERR_NULL_POINTER, "%s is NULL", e ? "e_total_host" : "plan");
+    return BQC_ERR_NULL_POINTER;
+  }
+  int dev = -1;
+  BQC_CUDA_OK(cudaGetDevice(&dev));
+  if (dev != e->device) {
+    set_error(BQC_ERR_DEVICE, "plan was created on device %d, current device is %d", e->device, dev);
+    return BQC_ERR_DEVICE;
+  }
+  if ((f_ov != nullptr) != (e->P.fock != 0)) {
+    set_error(BQC_ERR_INVALID_OPTION, "f_ov %s but the plan was created %s opts->f_ov", f_ov ? "given" : "NULL",
+              e->P.fock ? "with" : "without");
+    return BQC_ERR_INVALID_OPTION;
+  }
+  Inputs in = {eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, f_ov};
+  BQC_TRY(validate_inputs(e->nocc, e->nvir, e->naux, in));
+  if (e_triplet_dev) BQC_TRY(check_device_ptr(e_triplet_dev, "e_triplet_dev"));
+  if (e->P.na < 2) {
+    set_error(BQC_ERR_INVALID_OPTION, "plan over a single outer orbital has no triplets; use bqc_t_energy_ex");
+    return BQC_ERR_INVALID_OPTION;
+  }
+  return e->run(in, e_total_host, e_triplet_dev, static_cast<cudaStream_t>(stream));
+}
+
+void bqc_t_plan_destroy(bqc_t_plan plan) { delete reinterpret_cast<Engine*>(plan); }
+
+size_t bqc_t_plan_workspace_bytes(bqc_t_plan plan) {
+  return plan ? reinterpret_cast<Engine*>(plan)->P.total : 0;
 }
 
 int bqc_t_energy_host(int nocc, int nvir, int naux, const double* eps_occ, const double* eps_vir,
@@ -1191,7 +1012,7 @@ int bqc_t_energy_host(int nocc, int nvir, int naux, const double* eps_occ, const
   size_t h2d = 0;
   // An occupied window [lo,hi) of the ijk-driven schedule reads t2 only through rows t2[x,:,:,:], lo <= x < hi
   // (B~ rows, hole columns, Fock tiles): copy just that contiguous slice; the rest of the device buffer is
-  // never read.  The abc-driven schedule transposes all of t2 and takes the whole array.
+  // never read.  The abc-driven schedule reads t2[:,:,a,b] for the virtuals of its window: the whole array.
   size_t t2_first = 0, t2_count = elems[3];
   if (!abc) {
     int lo = 0, hi = nocc;
@@ -1238,6 +1059,20 @@ int bqc_t_energy_host(int nocc, int nvir, int naux, const double* eps_occ, const
   return rc;
 }
 
+// ---- single steps (parity tests): a private engine over the orbitals involved, one block --------------------
+static int debug_engine(Engine& e, int nocc, int nvir, int naux, const Inputs& in, const std::vector<int>& act,
+                        cudaStream_t stream) {
+  bqc_t_opts o2;
+  memset(&o2, 0, sizeof(o2));
+  o2.max_batch = 1;
+  o2.occ_block = (int)act.size();
+  BQC_TRY(e.init(nocc, nvir, naux, &o2, nullptr, 0, &act));
+  e.in = in;
+  e.s_main = stream;
+  BQC_TRY(e.prepare(stream));
+  return BQC_OK;
+}
+
 int bqc_t_debug_slabs(int nocc, int nvir, int naux, const double* t2, const double* B_oo, const double* B_ov,
                       const double* B_vv, int x, int y, double* I_dev, double* O_dev, double* J_dev,
                       void* stream_v) {
@@ -1253,43 +1088,38 @@ int bqc_t_debug_slabs(int nocc, int nvir, int naux, const double* t2, const doub
   BQC_TRY(check_device_ptr(B_oo, "B_oo"));
   BQC_TRY(check_device_ptr(B_ov, "B_ov"));
   BQC_TRY(check_device_ptr(B_vv, "B_vv"));
+  if (I_dev) BQC_TRY(check_device_ptr(I_dev, "I_dev"));
+  if (O_dev) BQC_TRY(check_device_ptr(O_dev, "O_dev"));
+  if (J_dev) BQC_TRY(check_device_ptr(J_dev, "J_dev"));
   Inputs in = {nullptr, nullptr, nullptr, t2, B_oo, B_ov, B_vv};
   std::vector<int> act;
   act.push_back(std::min(x, y));
   if (x != y) act.push_back(std::max(x, y));
-  bqc_t_opts o2;
-  memset(&o2, 0, sizeof(o2));
-  o2.max_batch = 1;
-  o2.occ_block = 2;
-  Pipeline p;
-  BQC_TRY(p.setup(nocc, nvir, naux, in, act, &o2, nullptr, 0, stream));
-  BQC_TRY(p.build_schedule());
-  p.actions.clear();
-  BQC_TRY(p.prepare());
-  Ctx& c = p.c;
-  const Plan& P = c.P;
+  Engine e;
+  BQC_TRY(debug_engine(e, nocc, nvir, naux, in, act, stream));
+  const Plan& P = e.P;
   const int px = (int)(std::find(act.begin(), act.end(), x) - act.begin());
   const int py = (int)(std::find(act.begin(), act.end(), y) - act.begin());
   const int v = nvir;
   if (I_dev) {
-    BQC_TRY(check_device_ptr(I_dev, "I_dev"));
-    BQC_TRY(p.form_block(0, 0, stream));   // one block holds all active orbitals (na <= 2 <= Bo)
-    BQC_TRY(launch_copy3(c.slabs() + (size_t)px * P.slab_elems, (long long)v * P.Kp, P.Kp, 1, I_dev, v, v, v,
+    BQC_TRY(e.exec_form(0, 0, stream));   // one block holds all active orbitals: slot = position
+    BQC_TRY(launch_copy3(e.slabs() + (size_t)px * P.slab_elems, (long long)v * P.Kp, P.Kp, 1, I_dev, v, v, v,
                          stream));
   }
-  if (O_dev) {
-    BQC_TRY(check_device_ptr(O_dev, "O_dev"));
-    // O_xy[l,u] = (x u|y l) = B~_xy[u, v + l]  -> out[l][u]
-    BQC_TRY(launch_copy3(c.btil() + ((size_t)px * P.na + py) * v * P.Kp + v, 0, 1, P.Kp, O_dev, 1, nocc, v,
-                         stream));
+  if (O_dev || J_dev) {
+    Action a;
+    memset(&a, 0, sizeof(a));
+    a.kind = Action::PAIR;
+    a.need_j = 1; a.need_panel = 1;
+    BQC_TRY(e.exec_pair(a, stream));
   }
-  if (J_dev) {
-    BQC_TRY(check_device_ptr(J_dev, "J_dev"));
-    BQC_CUDA_OK(cudaMemcpyAsync(J_dev, c.J() + ((size_t)px * P.na + py) * v * v, (size_t)v * v * 8,
+  if (O_dev)   // O_xy[l,u] = (x u|y l) = B~_xy[u, v + l]  -> out[l][u]
+    BQC_TRY(launch_copy3(e.btil() + ((size_t)px * P.nslots + py) * v * P.Kp + v, 0, 1, P.Kp, O_dev, 1, nocc, v,
+                         stream));
+  if (J_dev)
+    BQC_CUDA_OK(cudaMemcpyAsync(J_dev, e.J() + ((size_t)px * P.nslots + py) * v * v, (size_t)v * v * 8,
                                 cudaMemcpyDeviceToDevice, stream));
-  }
   BQC_CUDA_OK(cudaStreamSynchronize(stream));
-  BQC_CUDA_OK(cudaStreamSynchronize(c.s_form));
   return BQC_OK;
 }
 
@@ -1301,7 +1131,6 @@ int bqc_t_debug_wv(int nocc, int nvir, int naux, const double* eps_occ, const do
   cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
   Inputs in = {eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, f_ov};
   BQC_TRY(validate_inputs(nocc, nvir, naux, in));
-  if (f_ov) BQC_TRY(check_device_ptr(f_ov, "f_ov"));
   if (i < 0 || j < 0 || k < 0 || i >= nocc || j >= nocc || k >= nocc) {
     set_error(BQC_ERR_INVALID_SIZE, "triplet (%d,%d,%d) outside [0,%d)", i, j, k, nocc);
     return BQC_ERR_INVALID_SIZE;
@@ -1311,22 +1140,15 @@ int bqc_t_debug_wv(int nocc, int nvir, int naux, const double* eps_occ, const do
   std::vector<int> act = {i, j, k};
   std::sort(act.begin(), act.end());
   act.erase(std::unique(act.begin(), act.end()), act.end());
-  bqc_t_opts o2;
-  memset(&o2, 0, sizeof(o2));
-  o2.max_batch = 1;
-  o2.occ_block = 3;
-  Pipeline p;
-  BQC_TRY(p.setup(nocc, nvir, naux, in, act, &o2, nullptr, 0, stream));
-  Ctx& c = p.c;
-  const Plan& P = c.P;
-  // schedule: DF task slots as usual, then the three F tasks of (i,j,k) in the caller's order
-  BQC_TRY(p.build_schedule());
-  p.actions.clear();
+  Engine e;
+  BQC_TRY(debug_engine(e, nocc, nvir, naux, in, act, stream));
+  const Plan& P = e.P;
+  // the three F tasks of (i,j,k) in the caller's order (one block: slot = position in `act`)
   auto pos = [&](int x) { return (int)(std::find(act.begin(), act.end(), x) - act.begin()); };
   const int pi = pos(i), pj = pos(j), pk = pos(k);
-  const size_t task0 = c.tasks.size();
+  std::vector<GemmTask> ft;
   {
-    auto pair = [&](int pz, int py) { return pz * P.na + py; };
+    auto pair = [&](int pz, int py) { return pz * P.nslots + py; };
     auto f_task = [&](int px, int py, int pz, int cls) {
       GemmTask g;
       memset(&g, 0, sizeof(g));
@@ -1334,25 +1156,30 @@ int bqc_t_debug_wv(int nocc, int nvir, int naux, const double* eps_occ, const do
       g.term[0].a_idx = px; g.term[0].a_transposed = 0; g.term[0].b_idx = pair(pz, py);
       g.term[1].a_idx = py; g.term[1].a_transposed = 1; g.term[1].b_idx = pair(pz, px);
       g.c_off = (long long)(cls * P.fsz);
-      c.tasks.push_back(g);
+      ft.push_back(g);
     };
     f_task(pi, pj, pk, 0);
     f_task(pi, pk, pj, 1);
     f_task(pj, pk, pi, 2);
   }
-  BQC_TRY(p.prepare());
-  BQC_TRY(p.form_block(0, 0, stream));
+  // the engine's own schedule is not executed here: the three tasks go into chunk 0
+  BQC_CUDA_OK(cudaMemcpyAsync(e.tasks_dev(0), ft.data(), 3 * sizeof(GemmTask), cudaMemcpyHostToDevice, stream));
+  BQC_TRY(e.exec_form(0, 0, stream));
+  Action a;
+  memset(&a, 0, sizeof(a));
+  a.kind = Action::PAIR;
+  a.need_j = 1; a.need_panel = 1;
+  BQC_TRY(e.exec_pair(a, stream));
   GemmParams prm;
   memset(&prm, 0, sizeof(prm));
   prm.ntasks = 3;
-  prm.tasks = c.tasks_dev() + task0;
-  prm.C = c.F();
-  BQC_TRY(launch_f_gemm(c, prm, stream));
-  BQC_TRY(launch_assemble_wv(c.F(), P.nbv, nvir, c.J(), P.na, pi, pj, pk, t1 + (size_t)i * nvir,
+  prm.tasks = e.tasks_dev(0);
+  prm.C = e.F();
+  BQC_TRY(e.launch_f_gemm(prm, stream));
+  BQC_TRY(launch_assemble_wv(e.F(), P.nbv, nvir, e.J(), P.nslots, pi, pj, pk, t1 + (size_t)i * nvir,
                              t1 + (size_t)j * nvir, t1 + (size_t)k * nvir, t2, nocc, i, j, k, f_ov, W_dev, V_dev,
                              stream));
-  BQC_CUDA_OK(cudaStreamSynchronize(stream));
-  BQC_CUDA_OK(cudaStreamSynchronize(c.s_form));
+  BQC_CUDA_OK(cudaStreamSynchronize(stream));   // `ft` and the engine go out of scope
   return BQC_OK;
 }
 
