@@ -49,13 +49,17 @@ int make_tensor_map_f64(CUtensorMap* out, const void* base, const unsigned long 
 }
 
 int device_sm_count() {
-  static int sms = 0;
-  if (sms == 0) {
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
-    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+  // per device: a process may drive several GPUs (cudaSetDevice) through the same library
+  static int sms[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+  if (dev < 0 || dev >= 64) {
+    int n = 0;
+    return cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess ? n : 0;
   }
-  return sms;
+  if (sms[dev] == 0 && cudaDeviceGetAttribute(&sms[dev], cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return 0;
+  return sms[dev];
 }
 
 // Modelled relative time of an N extent covered by tiles of 8*nf columns: padded columns times a per-tile
@@ -128,17 +132,19 @@ int split_m(int m1_ext, int m2_ext, MSegment seg[2]) {
   return nbest;
 }
 
-template <int NF>
+template <int NF, bool kStaged>
 static int launch_nf(const CUtensorMap& tmA, const CUtensorMap& tmAT, const CUtensorMap& tmB,
                      const GemmParams& prm, int grid, cudaStream_t stream) {
-  static std::once_flag once;
-  static cudaError_t attr_err = cudaSuccess;
-  std::call_once(once, [] {
-    attr_err = cudaFuncSetAttribute(gemm_nt_kernel<NF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    gemm_smem_bytes(NF));
-  });
-  BQC_CUDA_OK(attr_err);
-  gemm_nt_kernel<NF><<<grid, kGemmThreads, gemm_smem_bytes(NF), stream>>>(tmA, tmAT, tmB, prm);
+  // the > 48 KiB dynamic shared memory opt-in is a per-device function attribute
+  static bool attr_set[64] = {};
+  int dev = 0;
+  BQC_CUDA_OK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64 || !attr_set[dev]) {
+    BQC_CUDA_OK(cudaFuncSetAttribute(gemm_nt_kernel<NF, kStaged>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     gemm_smem_bytes(NF, kStaged)));
+    if (dev >= 0 && dev < 64) attr_set[dev] = true;
+  }
+  gemm_nt_kernel<NF, kStaged><<<grid, kGemmThreads, gemm_smem_bytes(NF, kStaged), stream>>>(tmA, tmAT, tmB, prm);
   count_launch();
   BQC_CUDA_OK(cudaGetLastError());
   return BQC_OK;
@@ -154,8 +160,18 @@ int launch_gemm_nt(int nf, const CUtensorMap& tmA, const CUtensorMap& tmAT, cons
     return BQC_ERR_CUDA;
   }
   const int grid = (int)(total < sms ? total : sms);
+  // blocked (F-layout) output goes through the shared-memory staging tile and bulk stores; it needs whole
+  // 8-row groups of one m1 per fragment row block, i.e. tq >= 8 (always true: choose_m_tile / split_m)
+  const bool staged = prm.out_mode == 1;
+  if (staged && prm.tq_log2 < 3) {
+    set_error(BQC_ERR_INVALID_OPTION, "launch_gemm_nt: blocked output needs tq >= 8");
+    return BQC_ERR_INVALID_OPTION;
+  }
   switch (nf) {
-#define BQC_NF_CASE(n) case n: return launch_nf<n>(tmA, tmAT, tmB, prm, grid, stream)
+#define BQC_NF_CASE(n)                                                            \
+  case n:                                                                         \
+    return staged ? launch_nf<n, true>(tmA, tmAT, tmB, prm, grid, stream)         \
+                  : launch_nf<n, false>(tmA, tmAT, tmB, prm, grid, stream)
     BQC_NF_CASE(4); BQC_NF_CASE(5); BQC_NF_CASE(6); BQC_NF_CASE(7); BQC_NF_CASE(8); BQC_NF_CASE(9);
     BQC_NF_CASE(10); BQC_NF_CASE(11); BQC_NF_CASE(12); BQC_NF_CASE(13); BQC_NF_CASE(14); BQC_NF_CASE(15);
     BQC_NF_CASE(16);
