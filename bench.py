@@ -43,7 +43,8 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5,
-                    help="BASELINE.json configs[n-1], n = 1..5; 6-8 = cc-pVTZ/QZ-shaped inputs (SURVEY NEXT-2)")
+                    help="BASELINE.json configs[n-1], n = 1..5; 6-8 = cc-pVTZ/QZ-shaped inputs (SURVEY NEXT-2); "
+                         "9 = the paper's largest CCSD(T) size, 1 380 orbitals (use --schedule abc)")
     ap.add_argument("--schedule", default="ijk", choices=["ijk", "abc"],
                     help="ijk: occupied triplets outside, v^3 inside (default); abc: the paper's loop order, "
                          "virtual triples outside, o^3 inside (BQC_T_FLAG_ABC_DRIVEN)")
@@ -379,11 +380,13 @@ def main():
     inp = make_config(args.config)
     gen_s = time.perf_counter() - t0
     host = [torch.from_numpy(a) for a in inp.arrays()]
-    try:
-        host = [t.pin_memory() for t in host]          # e2e copies come from pinned memory
-        pinned = True
-    except RuntimeError:
-        pinned = False
+    pinned = False
+    if inp.nbytes() < 48e9:                             # a pinned second copy of 117 GB (config 9) does not fit the host
+        try:
+            host = [t.pin_memory() for t in host]      # e2e copies come from pinned memory
+            pinned = True
+        except RuntimeError:
+            pass
     dev = [t.cuda(non_blocking=True) for t in host]
     torch.cuda.synchronize()
     ws = torch.empty(bqc.bqc_t_workspace_bytes(o, v, X, opts), dtype=torch.uint8, device="cuda")
@@ -443,7 +446,8 @@ def main():
     # end to end through the C ABI with HOST buffers (H2D of all inputs + D2H of the scalar inside)
     e2e_ms, h2d, d2h = None, 0, 0
     if args.e2e_steps > 0:
-        del ws
+        del ws, dev                                     # the host-pointer call makes its own device copies
+        bqc.bqc_release_cached()
         torch.cuda.empty_cache()
         eopts = bqc.make_opts(occ_block=args.occ_block, occ_lo=opts.occ_lo, occ_hi=opts.occ_hi,
                               shard_rank=opts.shard_rank, shard_count=opts.shard_count,

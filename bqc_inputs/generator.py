@@ -15,6 +15,11 @@ Recipe (BASELINE.json `configs`, reading G12 of SURVEY.md §8(c)):
     6. only when ``f_std > 0`` (non-canonical reference):
        ``f_ov`` [nocc, nvir] N(0, f_std), drawn last so draws 1-5 do not change.
 * integrals are *defined* as (pq|rs) = sum_Q B[Q,p,q] B[Q,r,s]  (exact DF).
+* "sliced" recipe (config 9, the paper's largest CCSD(T) size, 117 GB of inputs): the same distributions and
+  symmetrisations, but every Q-slice of B and every t2[i] slab has its own PCG64 stream,
+  ``default_rng([seed, 1, q])`` / ``default_rng([seed, 3, i])`` (eps_occ, eps_vir, t1 from
+  ``default_rng([seed, 2])`` in that order), so that the slices can be drawn in parallel and B is never held
+  as one [naux, n, n] array.
 
 These are synthetic stand-ins shaped like the paper's water-cluster cc-pVDZ
 workloads (24 orbitals, 5 occupied per water).
@@ -63,6 +68,9 @@ CONFIGS = {
     6: dict(nocc=20, nvir=212, naux=812, t2_std=1e-2, seed=1006),    # 4 waters, cc-pVTZ-shaped
     7: dict(nocc=10, nvir=220, naux=805, t2_std=1e-2, seed=1007),    # 2 waters, cc-pVQZ-shaped
     8: dict(nocc=40, nvir=424, naux=1624, t2_std=5e-3, seed=1008),   # 8 waters, cc-pVTZ-shaped
+    # PAPER.md:381 "capable of handling up to 1 380 orbitals": 12 waters, cc-pVQZ-shaped (115 orbitals and
+    # 5 occupied per water), naux = 3.5 x orbitals.  117 GB of inputs: the sliced recipe above.
+    9: dict(nocc=60, nvir=1320, naux=4830, t2_std=5e-3, seed=1009, recipe="sliced"),
 }
 
 
@@ -104,10 +112,67 @@ def make_inputs(nocc: int, nvir: int, naux: int, seed: int,
                    name=name or f"o{nocc}v{nvir}x{naux}s{seed}", f_ov=f_ov)
 
 
+def _symmetrise_t2(t2: np.ndarray) -> None:
+    """t2 <- (G + G.transpose(1,0,3,2)) / 2 in place, without a second full-size copy."""
+    nocc = t2.shape[0]
+    for i in range(nocc):
+        for j in range(i, nocc):
+            if i == j:
+                blk = t2[i, i]
+                blk += blk.T.copy()
+                blk *= 0.5
+            else:
+                a = t2[i, j]
+                b = t2[j, i]
+                a += b.T
+                a *= 0.5
+                b[...] = a.T
+
+
+def make_inputs_sliced(nocc: int, nvir: int, naux: int, seed: int, t1_std: float = 1e-3,
+                       t2_std: float = 1e-2, b_std: float = 0.1, name: str = "", threads: int = 0) -> TInputs:
+    """The "sliced" recipe of the module docstring: one stream per Q-slice of B and per t2[i] slab, drawn by
+    a thread pool (NumPy releases the GIL while it fills), block arrays written in place."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    n = nocc + nvir
+    B_oo = np.empty((naux, nocc, nocc))
+    B_ov = np.empty((naux, nocc, nvir))
+    B_vv = np.empty((naux, nvir, nvir))
+
+    def b_slice(q):
+        g = np.random.default_rng([seed, 1, q]).normal(0.0, b_std, size=(n, n))
+        g += g.T.copy()
+        g *= 0.5
+        B_oo[q] = g[:nocc, :nocc]
+        B_ov[q] = g[:nocc, nocc:]
+        B_vv[q] = g[nocc:, nocc:]
+
+    t2 = np.empty((nocc, nocc, nvir, nvir))
+
+    def t2_slab(i):
+        t2[i] = np.random.default_rng([seed, 3, i]).normal(0.0, t2_std, size=(nocc, nvir, nvir))
+
+    with ThreadPoolExecutor(max_workers=threads or (os.cpu_count() or 1)) as ex:
+        list(ex.map(b_slice, range(naux)))
+        list(ex.map(t2_slab, range(nocc)))
+    rng = np.random.default_rng([seed, 2])
+    eps_occ = np.sort(rng.uniform(-1.5, -0.4, size=nocc))
+    eps_vir = np.sort(rng.uniform(0.15, 3.0, size=nvir))
+    t1 = rng.normal(0.0, t1_std, size=(nocc, nvir))
+    _symmetrise_t2(t2)
+    return TInputs(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv,
+                   name=name or f"o{nocc}v{nvir}x{naux}s{seed}sliced")
+
+
 def make_config(idx: int, **overrides) -> TInputs:
-    """BASELINE.json configs[idx-1] (idx = 1..5); idx = 6..8: the larger-basis shapes of NEXT-2."""
+    """BASELINE.json configs[idx-1] (idx = 1..5); idx = 6..8: the larger-basis shapes of NEXT-2; 9: the paper's
+    largest CCSD(T) size (sliced recipe)."""
     c = dict(CONFIGS[idx])
     c.update(overrides)
+    if c.get("recipe") == "sliced":
+        return make_inputs_sliced(c["nocc"], c["nvir"], c["naux"], c["seed"], t1_std=c.get("t1_std", 1e-3),
+                                  t2_std=c["t2_std"], name=f"config{idx}")
     return make_inputs(c["nocc"], c["nvir"], c["naux"], c["seed"],
                        t1_std=c.get("t1_std", 1e-3), t2_std=c["t2_std"],
                        name=f"config{idx}", f_std=c.get("f_std", 0.0))

@@ -72,6 +72,16 @@ def lib():
     L.bqc_t_workspace_bytes.argtypes = [c_int, c_int, c_int, POINTER(bqc_t_opts)]
     L.bqc_sum_in_order.restype = c_int
     L.bqc_sum_in_order.argtypes = [dp, c_size_t, POINTER(c_double), c_void_p]
+    L.bqc_release_cached.restype = None
+    L.bqc_release_cached.argtypes = []
+    L.bqc_t_plan_create.restype = c_int
+    L.bqc_t_plan_create.argtypes = [c_int] * 3 + [POINTER(bqc_t_opts), c_void_p, c_size_t, POINTER(c_void_p)]
+    L.bqc_t_plan_execute.restype = c_int
+    L.bqc_t_plan_execute.argtypes = [c_void_p] + [dp] * 8 + [POINTER(c_double), dp, c_void_p]
+    L.bqc_t_plan_destroy.restype = None
+    L.bqc_t_plan_destroy.argtypes = [c_void_p]
+    L.bqc_t_plan_workspace_bytes.restype = c_size_t
+    L.bqc_t_plan_workspace_bytes.argtypes = [c_void_p]
     L.bqc_last_error.restype = c_int
     L.bqc_error_string.restype = c_char_p
     L.bqc_error_string.argtypes = [c_int]
@@ -160,6 +170,13 @@ def make_opts(occ_block=0, occ_lo=0, occ_hi=0, shard_rank=0, shard_count=1, max_
     return o
 
 
+def _check_f_ov(opts, nocc, nvir, device):
+    """opts.f_ov (kept alive by make_opts) must be [nocc, nvir] in the memory space of the entry point."""
+    f = getattr(opts, "_f_ov_keepalive", None) if opts is not None else None
+    if f is not None:
+        _ptr(f, (nocc, nvir), "opts.f_ov", device)
+
+
 def _optp(opts):
     return byref(opts) if opts is not None else None
 
@@ -243,6 +260,7 @@ def bqc_t_energy_ex(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv
     `e_triplet`: optional float64 CUDA tensor [num_triplets] filled with e_ijk
     (e_abc over virtual triples, [num_triplets(nvir)], under BQC_T_FLAG_ABC_DRIVEN)."""
     p = _inputs(nocc, nvir, naux, (eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv), True)
+    _check_f_ov(opts, nocc, nvir, True)
     ws_ptr, ws_bytes = None, 0
     if workspace is not None:
         ws_ptr, ws_bytes = c_void_p(workspace.data_ptr()), workspace.numel() * workspace.element_size()
@@ -253,6 +271,47 @@ def bqc_t_energy_ex(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv
     _check(lib().bqc_t_energy_ex(nocc, nvir, naux, *p, _optp(opts), ws_ptr, ws_bytes, byref(e), et,
                                  _stream()))
     return e.value
+
+
+def bqc_release_cached():
+    lib().bqc_release_cached()
+
+
+class bqc_t_plan:
+    """Handle of bqc_t_plan_create / _execute / _destroy (include/bqc_t.h): marshalling only."""
+
+    def __init__(self, nocc, nvir, naux, opts=None, workspace=None):
+        self.nocc, self.nvir, self.naux, self.opts = nocc, nvir, naux, opts
+        self._ws = workspace                      # kept alive: the plan uses it until destroyed
+        ws_ptr, ws_bytes = None, 0
+        if workspace is not None:
+            ws_ptr, ws_bytes = c_void_p(workspace.data_ptr()), workspace.numel() * workspace.element_size()
+        self._h = c_void_p()
+        _check(lib().bqc_t_plan_create(nocc, nvir, naux, _optp(opts), ws_ptr, ws_bytes, byref(self._h)))
+
+    def workspace_bytes(self):
+        return lib().bqc_t_plan_workspace_bytes(self._h)
+
+    def execute(self, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv, f_ov=None, e_triplet=None):
+        p = _inputs(self.nocc, self.nvir, self.naux, (eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv), True)
+        f = _ptr(f_ov, (self.nocc, self.nvir), "f_ov", True) if f_ov is not None else None
+        et = None
+        if e_triplet is not None:
+            et = _ptr(e_triplet, (_ntrip_out(self.nocc, self.nvir, self.opts),), "e_triplet", True)
+        e = c_double(0.0)
+        _check(lib().bqc_t_plan_execute(self._h, *p, f, byref(e), et, _stream()))
+        return e.value
+
+    def destroy(self):
+        if self._h:
+            lib().bqc_t_plan_destroy(self._h)
+            self._h = c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
 
 
 def bqc_t_last_profile():
@@ -268,6 +327,7 @@ def bqc_t_energy_host(nocc, nvir, naux, eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_
                       e_triplet=None):
     """End-to-end call with HOST tensors.  Returns (E, h2d_bytes, d2h_bytes)."""
     p = _inputs(nocc, nvir, naux, (eps_occ, eps_vir, t1, t2, B_oo, B_ov, B_vv), False)
+    _check_f_ov(opts, nocc, nvir, False)
     et = None
     if e_triplet is not None:
         et = _ptr(e_triplet, (_ntrip_out(nocc, nvir, opts),), "e_triplet", False)

@@ -125,8 +125,24 @@ def test_single_occupied_is_exactly_zero():
     assert bqc.bqc_t_energy(*dims(inp), *to_device(inp)) == 0.0
 
 
-@pytest.mark.parametrize("cfg,count", [(2, 10), (3, 5)])
-def test_energy_sampled_triplets(cfg, count):
+def test_config2_full_energy_and_every_triplet():
+    """the full oracle on config 2 — E(T) and all 1 540 per-triplet values."""
+    inp = make_config(2)
+    d = to_device(inp)
+    o = inp.nocc
+    et = torch.empty(bqc.bqc_t_num_triplets(o), dtype=torch.float64, device="cuda")
+    e = bqc.bqc_t_energy_ex(*dims(inp), *d, e_triplet=et)
+    got = et.cpu().numpy()
+    e_ref, trip_ref = orc.t_energy(inp, return_triplets=True)
+    assert len(trip_ref) == 1540
+    assert abs(e - e_ref) <= e_tol(e_ref)
+    assert np.all(np.abs(got - trip_ref) <= 1e-10 * np.abs(trip_ref) + 1e-12 * abs(e_ref) / 1540)
+    assert bqc.bqc_t_energy(*dims(inp), *d) == e
+
+
+def test_config3_sixteen_seeded_triplets():
+    """a seeded subset of 16 triplets (seed 103) of config 3, plus any-size properties."""
+    cfg, count = 3, 16
     inp = make_config(cfg)
     d = to_device(inp)
     o = inp.nocc
@@ -167,10 +183,31 @@ def test_full_size_bench_configuration_sampled(cfg):
             assert got[idx] < 0.0
             inside += 1
     assert inside == 210 and np.count_nonzero(got) == 210        # nothing outside the window
-    for (i, j, k) in [(2, 2, 7), (0, 9, 9), (1, 4, 8)]:
+    # eight triplets of the window: the three classes by hand + a seeded draw (seed 40 + cfg)
+    rng = np.random.default_rng(40 + cfg)
+    trips = [(2, 2, 7), (0, 9, 9), (1, 4, 8)]
+    while len(trips) < 8:
+        t = tuple(sorted(int(x) for x in rng.integers(0, 10, size=3)))
+        if t not in trips and not (t[0] == t[1] == t[2]):
+            trips.append(t)
+    for (i, j, k) in trips:
         ref = orc.e_triplet(inp, i, j, k)
         g = got[bqc.bqc_t_triplet_index(o, i, j, k)]
         assert abs(g - ref) <= 1e-10 * abs(ref) + 1e-12 * abs(e) / 210, (i, j, k, g, ref)
+    if cfg == 4:
+        # one abc-driven sample at full size: a virtual window of 8, three virtual triples against the oracle's
+        # separately written abc loop
+        v = inp.nvir
+        aopts = bqc.make_opts(occ_lo=0, occ_hi=8, flags=bqc.BQC_T_FLAG_ABC_DRIVEN)
+        eta = torch.empty(bqc.bqc_t_num_triplets(v), dtype=torch.float64, device="cuda")
+        ea = bqc.bqc_t_energy_ex(*dims(inp), *d, opts=aopts, e_triplet=eta)
+        ga = eta.cpu().numpy()
+        assert np.count_nonzero(ga) == 8 * 9 * 10 // 6 - 8
+        for (a, b, c) in [(0, 3, 7), (2, 2, 5), (1, 6, 6)]:
+            ref = orc.e_virtual_triple(inp, a, b, c)
+            g = ga[bqc.bqc_t_triplet_index(v, a, b, c)]
+            assert abs(g - ref) <= 1e-10 * abs(ref) + 1e-12 * abs(ea) / 112, (a, b, c, g, ref)
+        del eta
     # single W / V elements straight from Eq. (2) (6 + 6 dot products), ragged tail included
     W, V = bqc.bqc_t_debug_wv(*dims(inp), *d, 1, 4, 8)
     v = inp.nvir

@@ -158,16 +158,28 @@ def test_w_and_v_elements_one_by_one(small):
             assert orc.v_element(small, i, j, k, a, b, c) == pytest.approx(V[a, b, c], rel=1e-11, abs=1e-17)
 
 
-# ---- P5: each slab is a plain matmul --------------------------------------
-def test_slabs_are_plain_matmuls(small):
-    X, o, v = small.naux, small.nocc, small.nvir
-    I1 = orc.slab_vvov(small, 1)
-    ref = (small.B_ov[:, 1, :].T @ small.B_vv.reshape(X, v * v)).reshape(v, v, v)
-    np.testing.assert_allclose(I1, ref, rtol=1e-13, atol=1e-16)
-    np.testing.assert_allclose(I1, I1.transpose(0, 2, 1), rtol=1e-12, atol=1e-16)
-    np.testing.assert_allclose(orc.slab_ooov(small, 1, 2), small.B_oo[:, 2, :].T @ small.B_ov[:, 1, :], rtol=1e-13)
-    np.testing.assert_allclose(orc.slab_ovov(small, 1, 2), small.B_ov[:, 1, :].T @ small.B_ov[:, 2, :], rtol=1e-13)
-    np.testing.assert_allclose(orc.slab_ovov(small, 1, 2), orc.slab_ovov(small, 2, 1).T, rtol=1e-13)
+# ---- P5: each slab against its definition written as explicit loops ---------
+def test_slabs_match_explicit_sums_over_Q():
+    """(pq|rs) = sum_Q B[Q,p,q] B[Q,r,s] written as plain Python loops on a tiny input (no library contraction:
+    a transposed operand or a wrong block in slab_* would fail here)."""
+    inp = make_inputs(3, 4, 5, seed=11)
+    X, o, v = inp.naux, inp.nocc, inp.nvir
+    x, y = 1, 2
+    I, O, J = orc.slab_vvov(inp, x), orc.slab_ooov(inp, x, y), orc.slab_ovov(inp, x, y)
+    for u in range(v):
+        for b in range(v):
+            for d in range(v):
+                ref = sum(inp.B_ov[Q, x, u] * inp.B_vv[Q, b, d] for Q in range(X))
+                assert I[u, b, d] == pytest.approx(ref, rel=1e-13, abs=1e-17)
+        for l in range(o):
+            ref = sum(inp.B_ov[Q, x, u] * inp.B_oo[Q, y, l] for Q in range(X))
+            assert O[l, u] == pytest.approx(ref, rel=1e-13, abs=1e-17)
+        for w in range(v):
+            ref = sum(inp.B_ov[Q, x, u] * inp.B_ov[Q, y, w] for Q in range(X))
+            assert J[u, w] == pytest.approx(ref, rel=1e-13, abs=1e-17)
+    # symmetries the definition implies
+    np.testing.assert_allclose(I, I.transpose(0, 2, 1), rtol=1e-12, atol=1e-16)
+    np.testing.assert_allclose(J, orc.slab_ovov(inp, y, x).T, rtol=1e-13)
 
 
 # ---- P3: invariants and special cases --------------------------------------
