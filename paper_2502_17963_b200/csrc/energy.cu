@@ -22,7 +22,11 @@ namespace {
 constexpr int kET = kVB;                      // 8
 constexpr int kEThreads = 256;
 constexpr int kTileElems = kET * kET * kET;   // 512
-constexpr int kJPitch = kET + 1;              // padded row pitch of the (ov|ov) tiles
+// (ov|ov) / t2 operand tiles: element (u, w) of an 8 x 8 tile sits at u*8 + (w ^ u).  The two lane patterns that
+// read them with 16 distinct addresses per half-warp — (u,w) = (y,z) and (z,y), z = 8 lanes, y = 2 values — then
+// hit 16 distinct 8-byte bank pairs (a padded pitch of 9 left one 2-way conflict in each: 15 % of the kernel's
+// shared wavefronts in the round-1 capture); the patterns through the warp-uniform x are broadcasts.
+__device__ __forceinline__ int jidx(int u, int w) { return (u << 3) | (w ^ u); }
 static_assert(kET == 8 && kEThreads == 256, "thread <-> element maps below assume 8^3 tiles and 256 threads");
 
 // the six permutations of three positions; 0-2 even (identity, two cyclic), 3-5 odd (transpositions)
@@ -30,12 +34,13 @@ __device__ constexpr int kPerm[6][3] = {{0, 1, 2}, {1, 2, 0}, {2, 0, 1}, {0, 2, 
 // index of the ordered pair (s,t), s != t, in the (ov|ov) tile array
 __device__ constexpr int kPairIdx[3][3] = {{-1, 0, 1}, {2, -1, 3}, {4, 5, -1}};
 
-// Shared-memory position of tile element (X, Y, Z): linear index with its low 4 bits (the 8-byte bank
+// Shared-memory position of W-tile element (X, Y, Z): linear index with its low 4 bits (the 8-byte bank
 // pair) XORed by a GF(2)-linear function of (X, Y>>1).  With this mask the 16 lanes of a half-warp hit 16
-// distinct bank pairs in every access pattern of the kernel: the three assembly passes (lanes vary along
+// distinct bank pairs in every access pattern of the W tiles: the three assembly passes (lanes vary along
 // w1,w2,v0,u0 of the F tile, written at (u,v,w), (u,w,v) and (w,u,v)) and the six permuted reads (lanes
 // vary along z and y0, read at every permutation of (x,y,z)).  The columns of the mask were found by
-// exhaustive search over all 2^20 linear maps.
+// exhaustive search over all 2^20 linear maps.  (The claim covers the W tiles only; the operand tiles of the
+// t1 / Fock terms have their own index map, jidx above.)
 __device__ __forceinline__ int sw(int X, int Y, int Z) {
   const int m = ((X & 1) * 9) ^ ((X & 2) << 1) ^ ((X & 4) >> 1) ^ ((Y & 2) << 1) ^ ((Y & 4) >> 1);
   return ((X << 6) | (Y << 3) | Z) ^ m;
@@ -43,7 +48,7 @@ __device__ __forceinline__ int sw(int X, int Y, int Z) {
 
 struct EnergySmem {
   double Wt[6][kTileElems];
-  double Jt[3][6][kET * kJPitch];   // [m][ordered block-position pair][local u * pitch + local w]
+  double Jt[3][6][kET * kET];       // [m][ordered block-position pair][jidx(local u, local w)]
   double t1s[3][3][kET];            // [which occupied (i,j,k)][block position][local]
   double epsv[3][kET];
   double red[kEThreads / 32];
@@ -51,7 +56,7 @@ struct EnergySmem {
 // extra operands of the non-canonical Fock term (Eqs. (5),(7), reading G15):
 // V += f[i,a] t2[j,k,b,c] + f[j,b] t2[i,k,a,c] + f[k,c] t2[i,j,a,b] — same shape as the t1 (ov|ov) term
 struct FockSmem {
-  double Tt[3][6][kET * kJPitch];   // t2[y,z] tiles, indexed like Jt
+  double Tt[3][6][kET * kET];       // t2[y,z] tiles, indexed like Jt
   double fs[3][3][kET];             // f_ov rows, indexed like t1s
 };
 struct NoSmem {};
@@ -125,7 +130,7 @@ __global__ void __launch_bounds__(kEThreads, kFock ? 3 : 4) energy_kernel(const 
       const int s = pr >> 1;
       const int t = (pr & 1) ? (s == 2 ? 1 : 2) : (s == 0 ? 1 : 0);
       const int gu = blk[s] * kET + lu, gw = blk[t] * kET + lw;
-      sm.Jt[m][pr][lu * kJPitch + lw] = (gu < v && gw < v) ? __ldg(Jm + (size_t)gu * v + gw) : 0.0;
+      sm.Jt[m][pr][jidx(lu, lw)] = (gu < v && gw < v) ? __ldg(Jm + (size_t)gu * v + gw) : 0.0;
       if constexpr (kFock) {
         // T^(0) = t2[j,k], T^(1) = t2[i,k], T^(2) = t2[i,j]
         const int ox = (m == 0) ? tr.j : tr.i;
@@ -134,7 +139,7 @@ __global__ void __launch_bounds__(kEThreads, kFock ? 3 : 4) energy_kernel(const 
         if (gu < v && gw < v)
           tval = a.dual ? -__ldg(a.t2 + (((size_t)gu * v + gw) * a.o + ox) * a.o + oy)   // -t2c[u,w,x,y]
                         : __ldg(a.t2 + (((size_t)ox * a.o + oy) * v + gu) * v + gw);
-        fk.Tt[m][pr][lu * kJPitch + lw] = tval;
+        fk.Tt[m][pr][jidx(lu, lw)] = tval;
       }
     }
   }
@@ -183,9 +188,9 @@ __global__ void __launch_bounds__(kEThreads, kFock ? 3 : 4) energy_kernel(const 
         for (int m = 0; m < 3; ++m) {
           const int sA = (m == 0) ? 1 : 0, sB = (m == 2) ? 1 : 2;
           const int pm = kPerm[p][m], pa = kPerm[p][sA], pb = kPerm[p][sB];
-          vp = fma(sm.t1s[m][pm][l[pm]], sm.Jt[m][kPairIdx[pa][pb]][l[pa] * kJPitch + l[pb]], vp);
+          vp = fma(sm.t1s[m][pm][l[pm]], sm.Jt[m][kPairIdx[pa][pb]][jidx(l[pa], l[pb])], vp);
           if constexpr (kFock)
-            vp = fma(fk.fs[m][pm][l[pm]], fk.Tt[m][kPairIdx[pa][pb]][l[pa] * kJPitch + l[pb]], vp);
+            vp = fma(fk.fs[m][pm][l[pm]], fk.Tt[m][kPairIdx[pa][pb]][jidx(l[pa], l[pb])], vp);
         }
       }
       // R at the permuted point = 3 w_p + (sum of same-parity w) - 2 (sum of opposite-parity w)   (Eq. (3))

@@ -40,14 +40,23 @@ struct Mp2Args {
   int i0, ni, o, v, ntp;
 };
 
-// grid: ((i - i0) * (o - i0) + (j - i0), tile pair); pairs with j < i exit at once
+// Pair slot p of a block of ni rows x nj columns counts the pairs il <= jl row by row: row il holds nj - il of
+// them.  Returns il and jl (ni is at most a few dozen: a short loop).
+__device__ __forceinline__ void pair_of_slot(int p, int nj, int* il, int* jl) {
+  int r = 0;
+  while (p >= nj - r) { p -= nj - r; ++r; }
+  *il = r;
+  *jl = r + p;
+}
+static long long pair_slots(int ni, int nj) { return (long long)ni * nj - (long long)ni * (ni - 1) / 2; }
+
+// grid: (pair slot il <= jl of the block, tile pair): only the pairs i <= j are launched
 __global__ void __launch_bounds__(kMThreads) mp2_pair_kernel(const Mp2Args a) {
   __shared__ double t1[kMT][kMT + 1];   // J[a in A][b in B]
   __shared__ double t2[kMT][kMT + 1];   // J[a in B][b in A]
   __shared__ double red[kMThreads / 32];
-  const int nj = a.o - a.i0;
-  const int il = blockIdx.x / nj, jl = blockIdx.x % nj;
-  if (jl < il) return;
+  int il, jl;
+  pair_of_slot(blockIdx.x, a.o - a.i0, &il, &jl);
   const int packed = a.tiles[blockIdx.y];
   const int A = packed & 0xffff, B = packed >> 16;
   const int v = a.v;
@@ -97,9 +106,8 @@ __global__ void __launch_bounds__(kMThreads) mp2_pair_kernel(const Mp2Args a) {
 __global__ void mp2_reduce_pairs_kernel(const double* __restrict__ partial, int ntp, int i0, int o,
                                         double* __restrict__ e_pair, double* __restrict__ e_w) {
   __shared__ double red[128];
-  const int nj = o - i0;
-  const int il = blockIdx.x / nj, jl = blockIdx.x % nj;
-  if (jl < il) return;
+  int il, jl;
+  pair_of_slot(blockIdx.x, o - i0, &il, &jl);
   const double* p = partial + (size_t)blockIdx.x * ntp;
   double s = 0.0;
   for (int n = threadIdx.x; n < ntp; n += 128) s += p[n];
@@ -263,6 +271,22 @@ static int mp2_impl(int o, int v, int X, const double* eps_occ, const double* ep
   BQC_TRY(launch_transpose_pad(B_ov, (long long)o * v, 0, (long long)o * v, bt, X, Xp, 0, 0, s));   // Bt_ov[(i,a)][Q], zero-padded to Xp
   ++nlaunch;
 
+  // The (ov|ov) sub-launches of a block alternate between the caller's stream and a helper stream: each is a
+  // persistent one-CTA-per-SM kernel of ~12 waves of tiles, so in one stream the partly filled last wave of every
+  // sub-launch (7 % of the time at config 5) would idle; on two streams the next sub-launch fills it.
+  struct Helper {
+    cudaStream_t s2 = nullptr;
+    cudaEvent_t ready = nullptr, done = nullptr;
+    ~Helper() {
+      if (ready) cudaEventDestroy(ready);
+      if (done) cudaEventDestroy(done);
+      if (s2) cudaStreamDestroy(s2);
+    }
+  } hp;
+  BQC_CUDA_OK(cudaStreamCreateWithFlags(&hp.s2, cudaStreamNonBlocking));
+  BQC_CUDA_OK(cudaEventCreateWithFlags(&hp.ready, cudaEventDisableTiming));
+  BQC_CUDA_OK(cudaEventCreateWithFlags(&hp.done, cudaEventDisableTiming));
+
   int ngemm = 0;
   const int nblk = ceil_div(o, Bi);
   for (int b = 0; b < nblk; ++b) {
@@ -274,7 +298,12 @@ static int mp2_impl(int o, int v, int X, const double* eps_occ, const double* ep
     // from ~15 % of the work (18-row blocks at config 5) to ~2 %.  grows keeps >= ~8 waves of tiles per launch.
     const int grows = std::max(2, std::min(Bi, (int)ceil(3.9e7 / ((double)o * v * v))));
     if (prof) BQC_TRY(sc_mem.mark(s));
+    // the helper stream may write the block buffer once the previous block's pair kernel has read it
+    BQC_CUDA_OK(cudaEventRecord(hp.ready, s));
+    BQC_CUDA_OK(cudaStreamWaitEvent(hp.s2, hp.ready, 0));
+    int sub = 0;
     for (int g0 = i0; g0 < i1; g0 += grows) {
+      cudaStream_t sg = (sub++ & 1) ? hp.s2 : s;
       const int g1 = std::min(i1, g0 + grows);
       const int M = (g1 - g0) * v;
       const long long N = (long long)(o - g0) * v;
@@ -304,16 +333,18 @@ static int mp2_impl(int o, int v, int X, const double* eps_occ, const double* ep
       prm.tasks = task_dev;
       // element (row (i - g0) v + a, column (j - g0) v + b) of this sub-launch -> Jblk[(i - i0) v + a][(j - i0) v + b]
       prm.C = jblk + (long long)(g0 - i0) * v * ld + (long long)(g0 - i0) * v;
-      BQC_TRY(launch_gemm_nt(nf, tA, tA, tB, prm, s));
+      BQC_TRY(launch_gemm_nt(nf, tA, tA, tB, prm, sg));
       ++nlaunch;
     }
+    BQC_CUDA_OK(cudaEventRecord(hp.done, hp.s2));
+    BQC_CUDA_OK(cudaStreamWaitEvent(s, hp.done, 0));
     if (prof) BQC_TRY(sc_mem.mark(s));
     ++ngemm;
 
     Mp2Args a;
     a.J = jblk; a.eps_occ = eps_occ; a.eps_vir = eps_vir; a.tiles = tiles; a.partial = partial;
     a.ld = ld; a.i0 = i0; a.ni = i1 - i0; a.o = o; a.v = v; a.ntp = ntp;
-    const int nslots = (i1 - i0) * (o - i0);
+    const int nslots = (int)pair_slots(i1 - i0, o - i0);
     mp2_pair_kernel<<<dim3(nslots, ntp), kMThreads, 0, s>>>(a);
     count_launch();
     BQC_CUDA_OK(cudaGetLastError());
