@@ -55,6 +55,9 @@ def parse():
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--peak-seconds", type=float, default=2.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-profile", action="store_true",
+                    help="time the calls without BQC_T_FLAG_PROFILE (the library then replays a CUDA graph for short "
+                         "schedules); the per-kernel split comes from one extra profiled call after the timed region")
     ap.add_argument("--cpu-triplets", type=int, default=3, help="triplets the oracle evaluates (cpu_baseline)")
     ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
                     help="torch.distributed backend of the N>1 plumbing (barrier, max-over-ranks, the scalar exchange)")
@@ -401,8 +404,14 @@ def main():
 
     e_trip = torch.zeros(bqc.bqc_t_num_triplets(nidx), dtype=torch.float64, device="cuda")
 
+    topts = opts
+    if args.no_profile:
+        topts = bqc.make_opts(occ_block=opts.occ_block, occ_lo=opts.occ_lo, occ_hi=opts.occ_hi,
+                              shard_rank=opts.shard_rank, shard_count=opts.shard_count,
+                              flags=opts.flags & ~bqc.BQC_T_FLAG_PROFILE)
+
     def step():
-        return bqc.bqc_t_energy_ex(o, v, X, *dev, opts=opts, workspace=ws, e_triplet=e_trip)
+        return bqc.bqc_t_energy_ex(o, v, X, *dev, opts=topts, workspace=ws, e_triplet=e_trip)
 
     for _ in range(args.warmup):
         e_val = step()
@@ -440,6 +449,9 @@ def main():
     else:
         ms = sum(a.elapsed_time(b) for a, b in pairs) / max(args.steps, 1)
         del flush
+    if args.no_profile:        # kernel split from one profiled call outside the timed region
+        assert bqc.bqc_t_energy_ex(o, v, X, *dev, opts=opts, workspace=ws, e_triplet=e_trip) == e_val
+        prof = dict(bqc.bqc_t_last_profile(), kernel_launches=prof["kernel_launches"])
     peak_after = bqc.bqc_fp64_peak_tflops(0, min(args.peak_seconds, 1.0))
     peak = max(peak_dmma, peak_after)
 
@@ -501,7 +513,10 @@ def main():
                                        "inputs replicated, one scalar exchange" if strong else
                                        f"{world} rank(s), one occupied window each, inputs replicated, one scalar exchange"),
                        "l2": l2_note,
-                       "timing": "CUDA events on the launch stream around K bqc_t_energy_ex calls, max over ranks",
+                       "timing": "CUDA events on the launch stream around K bqc_t_energy_ex calls, max over ranks"
+                                 + ("; timed without BQC_T_FLAG_PROFILE (CUDA-graph replay for short schedules), "
+                                    "kernel_ms_per_step / roofline from one profiled call after the timed region"
+                                    if args.no_profile else ""),
                        "pinned_host": pinned, "input_gen_s": round(gen_s, 1)},
             "pct_of_fp64_tensor_peak": 100.0 * value / (peak * world),
             "fp64_tensor_peak_tflops_measured": peak,

@@ -124,6 +124,12 @@ __device__ __forceinline__ double lds_f64(uint32_t addr) {
   return v;
 }
 
+// 16-byte st.shared with a 32-bit shared-window address (a generic-pointer store compiles to ST.E.128, which
+// goes through the generic address check).
+__device__ __forceinline__ void sts_v2_f64(uint32_t addr, double a, double b) {
+  asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(a), "d"(b) : "memory");
+}
+
 #endif  // __CUDACC__
 
 }  // namespace bqc

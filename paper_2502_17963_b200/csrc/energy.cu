@@ -92,79 +92,99 @@ __global__ void __launch_bounds__(kEThreads, kFock ? 3 : 4) energy_kernel(const 
   const int eu = ((tid >> 3) & 1) | (((tid >> 6) & 3) << 1);
   const int epair = ((eu << 6) | (ev << 3) | ew) >> 1;
 
-  auto load6 = [&](double2 (&val)[6], int phase) {
-#pragma unroll
-    for (int pi = 0; pi < 6; ++pi) {
-      const int P = blk[kPerm[pi][0]], Q = blk[kPerm[pi][1]], R = blk[kPerm[pi][2]];
-      const double* src = phase == 0 ? F1 + blk_off(nb, P, Q, R)
-                                     : (phase == 1 ? F2 + blk_off(nb, P, R, Q) : F3 + blk_off(nb, Q, R, P));
-      val[pi] = __ldcs(reinterpret_cast<const double2*>(src) + epair);   // read once: streaming, evict-first
+  // Orbits with repeated blocks (A == B and / or B == C) reach fewer than six distinct tiles: permutation pi
+  // then has the same block triple as an earlier one, canon_of(pi), and shares its W tile (neither loaded nor
+  // assembled twice).  In kPerm order — (A,B,C) (B,C,A) (C,A,B) (A,C,B) (C,B,A) (B,A,C), A <= B <= C — the
+  // distinct tiles are always the first nown = 6, 3 or 1 permutations.  CTA-uniform.
+  const bool eAB = blk[0] == blk[1], eBC = blk[1] == blk[2], eAll = eAB && eBC;
+  const int c1 = eAll ? 0 : 1, c2 = eAll ? 0 : 2, c3 = eAll ? 0 : (eAB ? 1 : (eBC ? 0 : 3)),
+            c4 = eAll ? 0 : (eAB ? 2 : (eBC ? 1 : 4)), c5 = eAll ? 0 : (eAB ? 0 : (eBC ? 2 : 5));
+  auto canon_of = [&](int pi) { return pi == 0 ? 0 : pi == 1 ? c1 : pi == 2 ? c2 : pi == 3 ? c3 : pi == 4 ? c4 : c5; };
+
+  // ---- small operands (issued while the tile loads fly): t1 rows, virtual orbital energies, (ov|ov) tiles
+  auto load_operands = [&]() {
+    if (tid < 3 * 3 * kET) {
+      const int l = tid & 7, pos = (tid >> 3) % 3, which = tid / (3 * kET);
+      const int occ = which == 0 ? tr.i : (which == 1 ? tr.j : tr.k);
+      const int av = blk[pos] * kET + l;
+      sm.t1s[which][pos][l] = (av < v) ? a.t1[(size_t)occ * v + av] : 0.0;
+      if constexpr (kFock) fk.fs[which][pos][l] = (av < v) ? a.f_ov[(size_t)occ * v + av] : 0.0;
+    } else if (tid < 3 * 3 * kET + 3 * kET) {
+      const int e = tid - 3 * 3 * kET;
+      const int l = e & 7, pos = e >> 3;
+      const int av = blk[pos] * kET + l;
+      sm.epsv[pos][l] = (av < v) ? a.eps_vir[av] : 1.0;
+    }
+    if (a.use_t1) {
+      for (int e = tid; e < 3 * 6 * kET * kET; e += kEThreads) {
+        const int lw = e & 7, lu = (e >> 3) & 7, pr = (e >> 6) % 6, m = e / (6 * kET * kET);
+        // J^(0) = J_jk, J^(1) = J_ik, J^(2) = J_ij
+        const int px = (m == 0) ? tr.pj : tr.pi;
+        const int py = (m == 2) ? tr.pj : tr.pk;
+        const double* Jm = a.J + ((size_t)px * a.nw + py) * v * v;
+        // pair index -> ordered block positions (s, t)
+        const int s = pr >> 1;
+        const int t = (pr & 1) ? (s == 2 ? 1 : 2) : (s == 0 ? 1 : 0);
+        const int gu = blk[s] * kET + lu, gw = blk[t] * kET + lw;
+        sm.Jt[m][pr][jidx(lu, lw)] = (gu < v && gw < v) ? __ldg(Jm + (size_t)gu * v + gw) : 0.0;
+        if constexpr (kFock) {
+          // T^(0) = t2[j,k], T^(1) = t2[i,k], T^(2) = t2[i,j]
+          const int ox = (m == 0) ? tr.j : tr.i;
+          const int oy = (m == 2) ? tr.j : tr.k;
+          double tval = 0.0;
+          if (gu < v && gw < v)
+            tval = a.dual ? -__ldg(a.t2 + (((size_t)gu * v + gw) * a.o + ox) * a.o + oy)   // -t2c[u,w,x,y]
+                          : __ldg(a.t2 + (((size_t)ox * a.o + oy) * v + gu) * v + gw);
+          fk.Tt[m][pr][jidx(lu, lw)] = tval;
+        }
+      }
     }
   };
 
-  double2 va[6], vb[6];
-  load6(va, 0);
-  load6(vb, 1);
-
-  // ---- small operands while the tile loads fly: t1 rows, virtual orbital energies, (ov|ov) tiles
-  if (tid < 3 * 3 * kET) {
-    const int l = tid & 7, pos = (tid >> 3) % 3, which = tid / (3 * kET);
-    const int occ = which == 0 ? tr.i : (which == 1 ? tr.j : tr.k);
-    const int av = blk[pos] * kET + l;
-    sm.t1s[which][pos][l] = (av < v) ? a.t1[(size_t)occ * v + av] : 0.0;
-    if constexpr (kFock) fk.fs[which][pos][l] = (av < v) ? a.f_ov[(size_t)occ * v + av] : 0.0;
-  } else if (tid < 3 * 3 * kET + 3 * kET) {
-    const int e = tid - 3 * 3 * kET;
-    const int l = e & 7, pos = e >> 3;
-    const int av = blk[pos] * kET + l;
-    sm.epsv[pos][l] = (av < v) ? a.eps_vir[av] : 1.0;
-  }
-  if (a.use_t1) {
-    for (int e = tid; e < 3 * 6 * kET * kET; e += kEThreads) {
-      const int lw = e & 7, lu = (e >> 3) & 7, pr = (e >> 6) % 6, m = e / (6 * kET * kET);
-      // J^(0) = J_jk, J^(1) = J_ik, J^(2) = J_ij
-      const int px = (m == 0) ? tr.pj : tr.pi;
-      const int py = (m == 2) ? tr.pj : tr.pk;
-      const double* Jm = a.J + ((size_t)px * a.nw + py) * v * v;
-      // pair index -> ordered block positions (s, t)
-      const int s = pr >> 1;
-      const int t = (pr & 1) ? (s == 2 ? 1 : 2) : (s == 0 ? 1 : 0);
-      const int gu = blk[s] * kET + lu, gw = blk[t] * kET + lw;
-      sm.Jt[m][pr][jidx(lu, lw)] = (gu < v && gw < v) ? __ldg(Jm + (size_t)gu * v + gw) : 0.0;
-      if constexpr (kFock) {
-        // T^(0) = t2[j,k], T^(1) = t2[i,k], T^(2) = t2[i,j]
-        const int ox = (m == 0) ? tr.j : tr.i;
-        const int oy = (m == 2) ? tr.j : tr.k;
-        double tval = 0.0;
-        if (gu < v && gw < v)
-          tval = a.dual ? -__ldg(a.t2 + (((size_t)gu * v + gw) * a.o + ox) * a.o + oy)   // -t2c[u,w,x,y]
-                        : __ldg(a.t2 + (((size_t)ox * a.o + oy) * v + gu) * v + gw);
-        fk.Tt[m][pr][jidx(lu, lw)] = tval;
+  // ---- load and assemble the first N W tiles: W[x,y,z] = F1[x,y,z] + F2[x,z,y] + F3[y,z,x]
+  // (F tile element (eu, ev, ew): F1 -> (x,y,z), F2 -> (x,z,y), F3 -> (y,z,x)); one code copy per N so that
+  // the per-tile values stay in registers
+  auto assemble = [&](auto NC) {
+    constexpr int N = decltype(NC)::value;
+    auto load_tiles = [&](double2 (&val)[N], int phase) {
+#pragma unroll
+      for (int pi = 0; pi < N; ++pi) {
+        const int P = blk[kPerm[pi][0]], Q = blk[kPerm[pi][1]], R = blk[kPerm[pi][2]];
+        const double* src = phase == 0 ? F1 + blk_off(nb, P, Q, R)
+                                       : (phase == 1 ? F2 + blk_off(nb, P, R, Q) : F3 + blk_off(nb, Q, R, P));
+        val[pi] = __ldcs(reinterpret_cast<const double2*>(src) + epair);   // read once: streaming, evict-first
       }
+    };
+    double2 va[N], vb[N];
+    load_tiles(va, 0);
+    load_tiles(vb, 1);
+    load_operands();
+#pragma unroll
+    for (int pi = 0; pi < N; ++pi) {
+      sm.Wt[pi][sw(eu, ev, ew)] = va[pi].x;
+      sm.Wt[pi][sw(eu, ev, ew + 1)] = va[pi].y;
     }
-  }
-
-  // ---- assemble the six W tiles: W[x,y,z] = F1[x,y,z] + F2[x,z,y] + F3[y,z,x]
-  // (F tile element (eu, ev, ew): F1 -> (x,y,z), F2 -> (x,z,y), F3 -> (y,z,x))
+    load_tiles(va, 2);   // va is free again: the third class flies across the barrier
+    __syncthreads();
 #pragma unroll
-  for (int pi = 0; pi < 6; ++pi) {
-    sm.Wt[pi][sw(eu, ev, ew)] = va[pi].x;
-    sm.Wt[pi][sw(eu, ev, ew + 1)] = va[pi].y;
-  }
-  load6(va, 2);        // va is free again: the third class flies across the barrier
-  __syncthreads();
+    for (int pi = 0; pi < N; ++pi) {
+      sm.Wt[pi][sw(eu, ew, ev)] += vb[pi].x;
+      sm.Wt[pi][sw(eu, ew + 1, ev)] += vb[pi].y;
+    }
+    __syncthreads();
 #pragma unroll
-  for (int pi = 0; pi < 6; ++pi) {
-    sm.Wt[pi][sw(eu, ew, ev)] += vb[pi].x;
-    sm.Wt[pi][sw(eu, ew + 1, ev)] += vb[pi].y;
-  }
-  __syncthreads();
-#pragma unroll
-  for (int pi = 0; pi < 6; ++pi) {
-    sm.Wt[pi][sw(ew, eu, ev)] += va[pi].x;
-    sm.Wt[pi][sw(ew + 1, eu, ev)] += va[pi].y;
-  }
-  __syncthreads();
+    for (int pi = 0; pi < N; ++pi) {
+      sm.Wt[pi][sw(ew, eu, ev)] += va[pi].x;
+      sm.Wt[pi][sw(ew + 1, eu, ev)] += va[pi].y;
+    }
+    __syncthreads();
+  };
+  if (eAll)
+    assemble(std::integral_constant<int, 1>{});
+  else if (eAB || eBC)
+    assemble(std::integral_constant<int, 3>{});
+  else
+    assemble(std::integral_constant<int, 6>{});
 
   // ---- points of this thread: z = tid & 7, y = (tid >> 3) & 7, x = (tid >> 6) + 4 r
   const int lz = tid & 7, ly = (tid >> 3) & 7, lx0 = tid >> 6;
@@ -175,7 +195,7 @@ __global__ void __launch_bounds__(kEThreads, kFock ? 3 : 4) energy_kernel(const 
     const int l[3] = {lx0 + 4 * r, ly, lz};
     double w[6];
 #pragma unroll
-    for (int p = 0; p < 6; ++p) w[p] = sm.Wt[p][sw(l[kPerm[p][0]], l[kPerm[p][1]], l[kPerm[p][2]])];
+    for (int p = 0; p < 6; ++p) w[p] = sm.Wt[canon_of(p)][sw(l[kPerm[p][0]], l[kPerm[p][1]], l[kPerm[p][2]])];
     const double se = w[0] + w[1] + w[2], so = w[3] + w[4] + w[5];
     const double re = se - 2.0 * so, ro = so - 2.0 * se;
     double s = 0.0;

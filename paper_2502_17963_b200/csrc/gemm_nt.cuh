@@ -178,12 +178,13 @@ __device__ __forceinline__ void gemm_consume(const GemmParams& prm, uint8_t* sme
       // 8 x 8 block of the 8^3-blocked F layout for a fixed m1 (tq >= 8): a contiguous 512-byte run, written
       // by one conflict-free warp-wide 16-byte store.  Run index = (row group, column block).
       mbar_wait(c_empty, c_phase ^ 1u);          // the store warp has read the previous tile out of staging
-      double* st = staging + ((size_t)((warp_m0 >> 3) * (kBN >> 3) + (warp_n0 >> 3)) << 6) + (g << 3) + 2 * t;
+      const uint32_t st = smem_u32(staging) +
+                          (uint32_t)(((((warp_m0 >> 3) * (kBN >> 3) + (warp_n0 >> 3)) << 6) + (g << 3) + 2 * t) << 3);
 #pragma unroll
       for (int i = 0; i < 4; ++i)
 #pragma unroll
         for (int j = 0; j < NFW; ++j)
-          *reinterpret_cast<double2*>(st + ((i * (kBN >> 3) + j) << 6)) = make_double2(acc[i][j][0], acc[i][j][1]);
+          sts_v2_f64(st + (uint32_t)((i * (kBN >> 3) + j) << 9), acc[i][j][0], acc[i][j][1]);
       fence_proxy_async();                       // generic-proxy writes -> visible to the bulk-copy engine
       __syncwarp();
       if (lane == 0) mbar_arrive(c_full);

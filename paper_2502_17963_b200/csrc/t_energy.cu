@@ -165,7 +165,7 @@ struct Engine {
   Inputs in;
   uint8_t* ws = nullptr;
   bool own_ws = false;
-  cudaStream_t s_main = nullptr, s_form = nullptr;
+  cudaStream_t s_main = nullptr, s_form = nullptr, s_cap = nullptr;
   cudaEvent_t ev_formed[4] = {}, ev_free[4] = {}, ev_fork = nullptr, ev_join = nullptr;
   bool ev_free_valid[4] = {};
   // F-GEMM configuration
@@ -182,7 +182,15 @@ struct Engine {
   std::vector<int> bt_owner;         // BQC_T_FLAG_SHARD_BLOCKS: owner of every block triple
   size_t ncompute = 0;               // W-builder launches of the whole schedule
   GemmTask df_task;                  // the one task of every DF GEMM (single term, c_off 0)
-  uint8_t* pinned = nullptr;         // 2 chunks: [chunk_trips TripletRec][3 chunk_trips GemmTask]
+  uint8_t* pinned = nullptr;         // 2 chunks: [chunk_trips TripletRec][3 chunk_trips GemmTask], then the
+                                     // orbit table and the DF task (static tables uploaded every call)
+  // CUDA graph of a short schedule (launch-bound regime): the whole call — repacking, slab and
+  // pair formation, W builder, energy kernels, sums — captured once per set of argument pointers and replayed
+  cudaGraphExec_t graph_exec = nullptr;
+  const void* graph_key[10] = {};
+  long long graph_launches = 0;
+  size_t ntriple_actions = 0;
+  bool capturing = false;
   cudaEvent_t ev_up[2] = {};         // upload of chunk b has executed: its pinned half may be rewritten
   bool ev_up_valid[2] = {};
   int chunk_next = 0;
@@ -222,6 +230,10 @@ struct Engine {
   GemmTask* tasks_dev(int b) const { return df_task_dev() + 8 + (size_t)b * 3 * P.chunk_trips; }
   TripletRec* trips_dev(int b) const { return reinterpret_cast<TripletRec*>(ws + P.off_trips) + (size_t)b * P.chunk_trips; }
   size_t pinned_chunk_bytes() const { return P.chunk_trips * (sizeof(TripletRec) + 3 * sizeof(GemmTask)); }
+  int* orbits_host() const { return reinterpret_cast<int*>(pinned + 2 * pinned_chunk_bytes()); }
+  GemmTask* df_task_host() const { return reinterpret_cast<GemmTask*>(pinned + 2 * pinned_chunk_bytes() + round_up((size_t)P.norbits * 4, 64)); }
+  bool graph_eligible() const { return !P.profile && ncompute <= 8 && ntriple_actions <= 2 && actions.size() <= 24; }
+  int enqueue(double* e_triplet_dev, cudaStream_t stream);
   TripletRec* trips_host(int b) const { return reinterpret_cast<TripletRec*>(pinned + (size_t)b * pinned_chunk_bytes()); }
   GemmTask* tasks_host(int b) const { return reinterpret_cast<GemmTask*>(trips_host(b) + P.chunk_trips); }
   // pipeline-space views of the small inputs (dual copies live in the workspace)
@@ -265,6 +277,7 @@ struct Engine {
     for (int b = 0; b < 2; ++b)
       if (ev_up[b]) cudaEventDestroy(ev_up[b]);
     if (s_form) cudaStreamDestroy(s_form);
+    if (graph_exec) cudaGraphExecDestroy(graph_exec);
     if (pinned) cudaFreeHost(pinned);
     if (own_ws && ws) cudaFree(ws);
   }
@@ -313,7 +326,7 @@ int Engine::init(int nocc_, int nvir_, int naux_, const bqc_t_opts* opts, void* 
   BQC_CUDA_OK(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
   BQC_CUDA_OK(cudaEventCreateWithFlags(&ev_join, cudaEventDisableTiming));
   for (int b = 0; b < 2; ++b) BQC_CUDA_OK(cudaEventCreateWithFlags(&ev_up[b], cudaEventDisableTiming));
-  BQC_CUDA_OK(cudaMallocHost(&pinned, 2 * pinned_chunk_bytes()));
+  BQC_CUDA_OK(cudaMallocHost(&pinned, 2 * pinned_chunk_bytes() + round_up((size_t)P.norbits * 4, 64) + sizeof(GemmTask)));
   df_task = single_term_task(0);
 
   const int v = P.v;
@@ -331,6 +344,8 @@ int Engine::init(int nocc_, int nvir_, int naux_, const bqc_t_opts* opts, void* 
   for (int A = 0; A < P.nbv; ++A)
     for (int B = A; B < P.nbv; ++B)
       for (int C = B; C < P.nbv; ++C) orbits.push_back(A | (B << 10) | (C << 20));
+  memcpy(orbits_host(), orbits.data(), orbits.size() * 4);
+  *df_task_host() = df_task;
   return build_schedule();
 }
 
@@ -373,6 +388,7 @@ int Engine::build_schedule() {
   const int Bo = P.Bo;
   actions.clear();
   ncompute = 0;
+  ntriple_actions = 0;
 
   // ---- block triples I <= J <= K with the slot-set protocol: I -> set 0, J -> set 1, K -> sets 2/3
   int set_block[4] = {-1, -1, -1, -1};
@@ -445,6 +461,7 @@ int Engine::build_schedule() {
             tg.bz = blks[p]; tg.by = blks[q]; tg.has_j = need_j;
           }
         actions.push_back(t);
+        ++ntriple_actions;
         ncompute += (ntr + P.nbatch - 1) / P.nbatch;
       }
     }
@@ -528,8 +545,8 @@ int Engine::prepare(cudaStream_t s) {
   BQC_CUDA_OK(cudaMemsetAsync(etrip(), 0, num_triplets(o) * 8, s));
   // the static tables: orbit table and the DF task (host copies live in the engine; the schedule chunks follow
   // block triple by block triple, see exec_triple)
-  BQC_CUDA_OK(cudaMemcpyAsync(orbits_dev(), orbits.data(), orbits.size() * 4, cudaMemcpyHostToDevice, s));
-  BQC_CUDA_OK(cudaMemcpyAsync(df_task_dev(), &df_task, sizeof(GemmTask), cudaMemcpyHostToDevice, s));
+  BQC_CUDA_OK(cudaMemcpyAsync(orbits_dev(), orbits_host(), orbits.size() * 4, cudaMemcpyHostToDevice, s));
+  BQC_CUDA_OK(cudaMemcpyAsync(df_task_dev(), df_task_host(), sizeof(GemmTask), cudaMemcpyHostToDevice, s));
   // the former stream starts after the repacked inputs exist
   BQC_CUDA_OK(cudaEventRecord(ev_fork, s));
   BQC_CUDA_OK(cudaStreamWaitEvent(s_form, ev_fork, 0));
@@ -620,12 +637,16 @@ int Engine::exec_compute(int chunk, size_t trip0, size_t ntrip, cudaStream_t s) 
 int Engine::exec_triple(const Action& a, cudaStream_t s) {
   const int b = chunk_next;
   chunk_next ^= 1;
-  if (ev_up_valid[b]) BQC_CUDA_OK(cudaEventSynchronize(ev_up[b]));   // the upload that last read this pinned half
+  // (while a graph is captured nothing executes: a captured schedule has at most two block triples, so each
+  // pinned half is written once and stays as the replayed copies need it)
+  if (!capturing && ev_up_valid[b]) BQC_CUDA_OK(cudaEventSynchronize(ev_up[b]));   // the upload that last read this half
   const size_t n = list_triple(a, trips_host(b), tasks_host(b));
   BQC_CUDA_OK(cudaMemcpyAsync(trips_dev(b), trips_host(b), n * sizeof(TripletRec), cudaMemcpyHostToDevice, s));
   BQC_CUDA_OK(cudaMemcpyAsync(tasks_dev(b), tasks_host(b), 3 * n * sizeof(GemmTask), cudaMemcpyHostToDevice, s));
-  BQC_CUDA_OK(cudaEventRecord(ev_up[b], s));
-  ev_up_valid[b] = true;
+  if (!capturing) {
+    BQC_CUDA_OK(cudaEventRecord(ev_up[b], s));
+    ev_up_valid[b] = true;
+  }
   for (size_t t0 = 0; t0 < n; t0 += P.nbatch)
     BQC_TRY(exec_compute(b, t0, std::min(n - t0, (size_t)P.nbatch), s));
   return BQC_OK;
@@ -682,6 +703,23 @@ int denominator_error(double emax, double vmin) {
   return BQC_ERR_DENOMINATOR;
 }
 
+// Everything of one evaluation that is enqueued on the stream(s), from the first memset to the last sum.
+int Engine::enqueue(double* e_triplet_dev, cudaStream_t stream) {
+  const bool prof = P.profile != 0;
+  const bool check_first = ncompute > 64;
+  // esum: [0] E, [1] denominator verdict (0 ok), [2] max eps_occ, [3] min eps_vir
+  BQC_CUDA_OK(cudaMemsetAsync(esum(), 0, 32, stream));
+  if (!check_first) BQC_TRY(launch_denominator_check(in.eps_occ, nocc, in.eps_vir, nvir, esum() + 1, stream));
+  BQC_TRY(prepare(stream));
+  if (prof) BQC_CUDA_OK(cudaEventRecord(prof_prepared, stream));
+  BQC_TRY(execute());
+  BQC_TRY(launch_final_sum(etrip(), (long long)num_triplets(P.o), esum(), stream));
+  if (prof) BQC_CUDA_OK(cudaEventRecord(prof_end, stream));
+  if (e_triplet_dev)
+    BQC_CUDA_OK(cudaMemcpyAsync(e_triplet_dev, etrip(), num_triplets(P.o) * 8, cudaMemcpyDeviceToDevice, stream));
+  return BQC_OK;
+}
+
 int Engine::run(const Inputs& inputs, double* e_total_host, double* e_triplet_dev, cudaStream_t stream) {
   in = inputs;
   s_main = stream;
@@ -711,16 +749,45 @@ int Engine::run(const Inputs& inputs, double* e_total_host, double* e_triplet_de
     }
     BQC_CUDA_OK(cudaEventRecord(prof_begin, stream));
   }
-  // esum: [0] E, [1] denominator verdict (0 ok), [2] max eps_occ, [3] min eps_vir
-  BQC_CUDA_OK(cudaMemsetAsync(esum(), 0, 32, stream));
-  if (!check_first) BQC_TRY(launch_denominator_check(in.eps_occ, nocc, in.eps_vir, nvir, esum() + 1, stream));
-  BQC_TRY(prepare(stream));
-  if (prof) BQC_CUDA_OK(cudaEventRecord(prof_prepared, stream));
-  BQC_TRY(execute());
-  BQC_TRY(launch_final_sum(etrip(), (long long)num_triplets(P.o), esum(), stream));
-  if (prof) BQC_CUDA_OK(cudaEventRecord(prof_end, stream));
-  if (e_triplet_dev)
-    BQC_CUDA_OK(cudaMemcpyAsync(e_triplet_dev, etrip(), num_triplets(P.o) * 8, cudaMemcpyDeviceToDevice, stream));
+  if (graph_eligible()) {
+    // Short schedule: replay the captured graph when the argument pointers repeat, else (re)capture it.
+    const void* key[10] = {in.eps_occ, in.eps_vir, in.t1, in.t2, in.B_oo, in.B_ov, in.B_vv, in.f_ov, e_triplet_dev,
+                           this};
+    if (!graph_exec || memcmp(key, graph_key, sizeof(key)) != 0) {
+      if (graph_exec) { cudaGraphExecDestroy(graph_exec); graph_exec = nullptr; }
+      // the pinned chunks must be quiescent before they are rewritten for the capture
+      for (int b = 0; b < 2; ++b)
+        if (ev_up_valid[b]) { BQC_CUDA_OK(cudaEventSynchronize(ev_up[b])); ev_up_valid[b] = false; }
+      chunk_next = 0;
+      cudaGraph_t graph = nullptr;
+      // captured on an internal stream (the caller's may be the legacy default stream, which cannot capture);
+      // the instantiated graph is launched on the caller's stream
+      if (!s_cap) BQC_CUDA_OK(cudaStreamCreateWithFlags(&s_cap, cudaStreamNonBlocking));
+      BQC_CUDA_OK(cudaStreamBeginCapture(s_cap, cudaStreamCaptureModeRelaxed));
+      capturing = true;
+      s_main = s_cap;
+      const int rc = enqueue(e_triplet_dev, s_cap);
+      s_main = stream;
+      capturing = false;
+      const cudaError_t ce = cudaStreamEndCapture(s_cap, &graph);
+      if (rc != BQC_OK) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        return rc;
+      }
+      BQC_CUDA_OK(ce);
+      const cudaError_t ie = cudaGraphInstantiate(&graph_exec, graph, 0);
+      cudaGraphDestroy(graph);
+      BQC_CUDA_OK(ie);
+      memcpy(graph_key, key, sizeof(key));
+      graph_launches = g_launches - launches0;
+    } else {
+      g_launches += graph_launches;   // the replay launches the same kernels
+    }
+    BQC_CUDA_OK(cudaGraphLaunch(graph_exec, stream));
+  } else {
+    BQC_TRY(enqueue(e_triplet_dev, stream));
+  }
   double res[4] = {0, 0, 0, 0};
   BQC_CUDA_OK(cudaMemcpyAsync(res, esum(), 32, cudaMemcpyDeviceToHost, stream));
   BQC_CUDA_OK(cudaStreamSynchronize(stream));   // joins s_form too (ev_join)

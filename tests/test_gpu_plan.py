@@ -127,3 +127,39 @@ def test_largest_shape_of_the_paper_runs_within_one_b200():
         ref = orc.e_virtual_triple(inp, a, b, cc)
         assert abs(g - ref) <= 1e-10 * abs(ref) + 1e-12 * abs(e) / ntr, (a, b, cc, g, ref)
     bqc.bqc_release_cached()
+
+
+def test_graph_replay_of_short_schedules_matches_the_eager_path():
+    """Short schedules without BQC_T_FLAG_PROFILE are captured into a CUDA graph and replayed when the argument
+    pointers repeat (the launch-bound regime).  Replays must track the VALUES behind the pointers,
+    re-capture when a pointer changes, and give the same bits as the eager (profiled) path."""
+    inp = make_config(1, t1_std=0.05)
+    d = to_device(inp)
+    n = bqc.bqc_t_num_triplets(inp.nocc)
+    et = torch.empty(n, dtype=torch.float64, device="cuda")
+    eager = torch.empty_like(et)
+    e_eager = bqc.bqc_t_energy_ex(*dims(inp), *d, opts=bqc.make_opts(flags=bqc.BQC_T_FLAG_PROFILE), e_triplet=eager)
+    e_ref = orc.t_energy(inp)
+    assert abs(e_eager - e_ref) <= e_tol(e_ref)
+    for _ in range(3):                                   # capture, then two replays
+        et.zero_()
+        assert bqc.bqc_t_energy_ex(*dims(inp), *d, e_triplet=et) == e_eager
+        assert torch.equal(et, eager)
+    # new values behind the same pointers: the replay recomputes everything
+    other = make_config(1, t1_std=0.05, seed=4242)
+    for dst, src in zip(d, to_device(other)):
+        dst.copy_(src)
+    e2 = bqc.bqc_t_energy_ex(*dims(inp), *d, e_triplet=et)
+    e2_ref = orc.t_energy(other)
+    assert abs(e2 - e2_ref) <= e_tol(e2_ref) and e2 != e_eager
+    # a different output pointer (and none at all): re-capture, same result
+    et2 = torch.empty_like(et)
+    assert bqc.bqc_t_energy_ex(*dims(inp), *d, e_triplet=et2) == e2 and torch.equal(et, et2)
+    assert bqc.bqc_t_energy_ex(*dims(inp), *d) == e2
+    assert bqc.bqc_t_energy(*dims(inp), *d) == e2
+    # a vanishing denominator is still reported (the verdict travels with the result)
+    d[1][0] = -2.0
+    with pytest.raises(bqc.BqcError) as ei:
+        bqc.bqc_t_energy_ex(*dims(inp), *d)
+    assert ei.value.code == 8
+    bqc.bqc_release_cached()
