@@ -508,6 +508,8 @@ def main():
             "scaling": "strong" if strong else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args.config, c, lo, hi, args.full, ntrip, abc),
+                       "sample": f"all {ntrip} triplets of the workload per step and GPU (the reference arm's step is one "
+                                 "triplet of the same workload; TFLOP/s normalises both)",
                        "schedule": args.schedule, "triplets_per_gpu": ntrip, "occ_block": bqc.bqc_t_plan_occ_block(o, v, X, opts),
                        "parallelism": (f"one E(T) dealt over {world} ranks by whole block triples (BQC_T_FLAG_SHARD_BLOCKS), "
                                        "inputs replicated, one scalar exchange" if strong else
