@@ -62,7 +62,7 @@ struct FockSmem {
 struct NoSmem {};
 
 __device__ __forceinline__ size_t blk_off(int nb, int P, int Q, int R) {
-  return (((size_t)P * nb + Q) * nb + R) * kTileElems;
+  return (size_t)((P * nb + Q) * nb + R) * kTileElems;   // nb <= 1023: the block number fits 32 bits
 }
 
 }  // namespace
@@ -116,28 +116,51 @@ __global__ void __launch_bounds__(kEThreads, kFock ? 3 : 4) energy_kernel(const 
       sm.epsv[pos][l] = (av < v) ? a.eps_vir[av] : 1.0;
     }
     if (a.use_t1) {
-      for (int e = tid; e < 3 * 6 * kET * kET; e += kEThreads) {
-        const int lw = e & 7, lu = (e >> 3) & 7, pr = (e >> 6) % 6, m = e / (6 * kET * kET);
-        // J^(0) = J_jk, J^(1) = J_ik, J^(2) = J_ij
-        const int px = (m == 0) ? tr.pj : tr.pi;
-        const int py = (m == 2) ? tr.pj : tr.pk;
-        const double* Jm = a.J + ((size_t)px * a.nw + py) * v * v;
-        // pair index -> ordered block positions (s, t)
-        const int s = pr >> 1;
-        const int t = (pr & 1) ? (s == 2 ? 1 : 2) : (s == 0 ? 1 : 0);
-        const int gu = blk[s] * kET + lu, gw = blk[t] * kET + lw;
-        sm.Jt[m][pr][jidx(lu, lw)] = (gu < v && gw < v) ? __ldg(Jm + (size_t)gu * v + gw) : 0.0;
-        if constexpr (kFock) {
-          // T^(0) = t2[j,k], T^(1) = t2[i,k], T^(2) = t2[i,j]
-          const int ox = (m == 0) ? tr.j : tr.i;
-          const int oy = (m == 2) ? tr.j : tr.k;
-          double tval = 0.0;
-          if (gu < v && gw < v)
-            tval = a.dual ? -__ldg(a.t2 + (((size_t)gu * v + gw) * a.o + ox) * a.o + oy)   // -t2c[u,w,x,y]
-                          : __ldg(a.t2 + (((size_t)ox * a.o + oy) * v + gu) * v + gw);
-          fk.Tt[m][pr][jidx(lu, lw)] = tval;
+      // 18 operand tiles (3 matrices x 6 ordered block-position pairs) of 64 elements: a thread owns element
+      // (lu, lw) = tid & 63 of the tiles g = (tid >> 6) + 4 it.  All loads are issued before the first store.
+      const int lw = tid & 7, lu = (tid >> 3) & 7, g0 = tid >> 6;
+      // (two rounds — tiles g0 + 0, 4, 8 and g0 + 12, 16 — so that the values in flight fit the register budget
+      // next to the twelve F-tile loads)
+      auto fill = [&](auto IT0, auto IT1) {
+        constexpr int it0 = decltype(IT0)::value, it1 = decltype(IT1)::value;
+        double jv[it1 - it0], tv[it1 - it0];
+#pragma unroll
+        for (int it = it0; it < it1; ++it) {
+          const int g = g0 + 4 * it;
+          jv[it - it0] = 0.0;
+          tv[it - it0] = 0.0;
+          if (g < 18) {
+            const int m = g / 6, pr = g - 6 * m;
+            // J^(0) = J_jk, J^(1) = J_ik, J^(2) = J_ij; pair index -> ordered block positions (s, t)
+            const int px = (m == 0) ? tr.pj : tr.pi;
+            const int py = (m == 2) ? tr.pj : tr.pk;
+            const int s = pr >> 1;
+            const int t = (pr & 1) ? (s == 2 ? 1 : 2) : (s == 0 ? 1 : 0);
+            const int gu = blk[s] * kET + lu, gw = blk[t] * kET + lw;
+            if (gu < v && gw < v) {
+              jv[it - it0] = __ldg(a.J + ((size_t)(px * a.nw + py) * v + gu) * v + gw);
+              if constexpr (kFock) {
+                // T^(0) = t2[j,k], T^(1) = t2[i,k], T^(2) = t2[i,j]
+                const int ox = (m == 0) ? tr.j : tr.i;
+                const int oy = (m == 2) ? tr.j : tr.k;
+                tv[it - it0] = a.dual ? -__ldg(a.t2 + (((size_t)gu * v + gw) * a.o + ox) * a.o + oy)   // -t2c[u,w,x,y]
+                                      : __ldg(a.t2 + (((size_t)ox * a.o + oy) * v + gu) * v + gw);
+              }
+            }
+          }
         }
-      }
+#pragma unroll
+        for (int it = it0; it < it1; ++it) {
+          const int g = g0 + 4 * it;
+          if (g < 18) {
+            const int m = g / 6, pr = g - 6 * m;
+            sm.Jt[m][pr][jidx(lu, lw)] = jv[it - it0];
+            if constexpr (kFock) fk.Tt[m][pr][jidx(lu, lw)] = tv[it - it0];
+          }
+        }
+      };
+      fill(std::integral_constant<int, 0>{}, std::integral_constant<int, 3>{});
+      fill(std::integral_constant<int, 3>{}, std::integral_constant<int, 5>{});
     }
   };
 
@@ -190,36 +213,64 @@ __global__ void __launch_bounds__(kEThreads, kFock ? 3 : 4) energy_kernel(const 
   const int lz = tid & 7, ly = (tid >> 3) & 7, lx0 = tid >> 6;
   const double dijk = a.eps_occ[tr.i] + a.eps_occ[tr.j] + a.eps_occ[tr.k];
   double acc = 0.0;
+  {
+    // The two points of a thread differ in one bit of x (x and x ^ 4).  Both index maps are GF(2)-linear, so
+    // every shared-memory index of the second point is the first point's XOR a compile-time constant that only
+    // depends on the slot x occupies after the permutation; operands that do not involve x are loaded once.
+    const int l[3] = {lx0, ly, lz};
+    double w0[6], w1[6];
 #pragma unroll
-  for (int r = 0; r < 2; ++r) {
-    const int l[3] = {lx0 + 4 * r, ly, lz};
-    double w[6];
-#pragma unroll
-    for (int p = 0; p < 6; ++p) w[p] = sm.Wt[canon_of(p)][sw(l[kPerm[p][0]], l[kPerm[p][1]], l[kPerm[p][2]])];
-    const double se = w[0] + w[1] + w[2], so = w[3] + w[4] + w[5];
-    const double re = se - 2.0 * so, ro = so - 2.0 * se;
-    double s = 0.0;
+    for (int p = 0; p < 6; ++p) {
+      const int i0 = sw(l[kPerm[p][0]], l[kPerm[p][1]], l[kPerm[p][2]]);
+      // flipping bit 2 of X / Y / Z moves sw() by 256^2 / 32^2 / 4 (the mask takes (X&4)>>1 and (Y&4)>>1)
+      const int dx = kPerm[p][0] == 0 ? 258 : (kPerm[p][1] == 0 ? 34 : 4);
+      const double* Wp = sm.Wt[canon_of(p)];
+      w0[p] = Wp[i0];
+      w1[p] = Wp[i0 ^ dx];
+    }
+    const double se0 = w0[0] + w0[1] + w0[2], so0 = w0[3] + w0[4] + w0[5];
+    const double re0 = se0 - 2.0 * so0, ro0 = so0 - 2.0 * se0;
+    const double se1 = w1[0] + w1[1] + w1[2], so1 = w1[3] + w1[4] + w1[5];
+    const double re1 = se1 - 2.0 * so1, ro1 = so1 - 2.0 * se1;
+    double s0 = 0.0, s1 = 0.0;
 #pragma unroll
     for (int p = 0; p < 6; ++p) {
       // V at the permuted point: W + t1[i,a](jb|kc) + t1[j,b](ia|kc) + t1[k,c](ia|jb)   (Eqs. (6),(7))
-      double vp = w[p];
+      double v0 = w0[p], v1 = w1[p];
       if (a.use_t1) {
 #pragma unroll
         for (int m = 0; m < 3; ++m) {
           const int sA = (m == 0) ? 1 : 0, sB = (m == 2) ? 1 : 2;
           const int pm = kPerm[p][m], pa = kPerm[p][sA], pb = kPerm[p][sB];
-          vp = fma(sm.t1s[m][pm][l[pm]], sm.Jt[m][kPairIdx[pa][pb]][jidx(l[pa], l[pb])], vp);
-          if constexpr (kFock)
-            vp = fma(fk.fs[m][pm][l[pm]], fk.Tt[m][kPairIdx[pa][pb]][jidx(l[pa], l[pb])], vp);
+          const int ji = jidx(l[pa], l[pb]);
+          const int dj = pa == 0 ? 36 : (pb == 0 ? 4 : 0);   // jidx(u ^ 4, w) = jidx ^ 36, jidx(u, w ^ 4) = jidx ^ 4
+          const double* t1m = sm.t1s[m][pm];
+          const double* Jm = sm.Jt[m][kPairIdx[pa][pb]];
+          const double ta = t1m[l[pm]], ja = Jm[ji];
+          const double tb = pm == 0 ? t1m[l[pm] + 4] : ta;
+          const double jb = dj ? Jm[ji ^ dj] : ja;
+          v0 = fma(ta, ja, v0);
+          v1 = fma(tb, jb, v1);
+          if constexpr (kFock) {
+            const double* fm = fk.fs[m][pm];
+            const double* Tm = fk.Tt[m][kPairIdx[pa][pb]];
+            const double fa = fm[l[pm]], qa = Tm[ji];
+            const double fb = pm == 0 ? fm[l[pm] + 4] : fa;
+            const double qb = dj ? Tm[ji ^ dj] : qa;
+            v0 = fma(fa, qa, v0);
+            v1 = fma(fb, qb, v1);
+          }
         }
       }
       // R at the permuted point = 3 w_p + (sum of same-parity w) - 2 (sum of opposite-parity w)   (Eq. (3))
-      s += (3.0 * w[p] + (p < 3 ? re : ro)) * vp;
+      s0 += (3.0 * w0[p] + (p < 3 ? re0 : ro0)) * v0;
+      s1 += (3.0 * w1[p] + (p < 3 ? re1 : ro1)) * v1;
     }
     // denominator (Eq. (3)) in registers
-    const bool valid = (blk[0] * kET + l[0] < v) && (blk[1] * kET + ly < v) && (blk[2] * kET + lz < v);
-    const double d = dijk - sm.epsv[0][l[0]] - sm.epsv[1][ly] - sm.epsv[2][lz];
-    if (valid) acc += s / d;
+    const bool valid_yz = (blk[1] * kET + ly < v) && (blk[2] * kET + lz < v);
+    const double ey = sm.epsv[1][ly], ez = sm.epsv[2][lz];
+    if (valid_yz && blk[0] * kET + lx0 < v) acc += s0 / (dijk - sm.epsv[0][lx0] - ey - ez);
+    if (valid_yz && blk[0] * kET + lx0 + 4 < v) acc += s1 / (dijk - sm.epsv[0][lx0 + 4] - ey - ez);
   }
   // multiplicity of the block triple under permutation (1, 2 or 6)
   const int same = (blk[0] == blk[1]) + (blk[1] == blk[2]);
