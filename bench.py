@@ -64,6 +64,10 @@ def parse():
     ap.add_argument("--share-gpu", action="store_true",
                     help="TEST ONLY: every rank uses cuda:0 (implies --backend gloo); exercises the N>1 code path on a "
                          "1-GPU box, its timings mean nothing and the line says so")
+    ap.add_argument("--shard-sweep", type=int, default=0, metavar="N",
+                    help="ONE GPU: evaluate the N block-triple shards of a full E(T) one after another and report "
+                         "each shard's time, flops and slab blocks formed, plus the strong-scaling efficiency they "
+                         "imply (T_1 / (N max_r T_r)); a projection from measured per-shard times, not an N-GPU run")
     ap.add_argument("--path", default="t", choices=["t", "mp2"],
                     help="t: the (T) energy (the headline); mp2: the DF-MP2 energy of PAPER.md Eq. (1) (SURVEY NEXT-4)")
     return ap.parse_args()
@@ -224,6 +228,12 @@ def run_reference(args, rank, world):
     print(json.dumps(out), flush=True)
 
 
+def pipe_peak_tflops(gpu=0):
+    """SMs x maximum SM clock x 128 FP64 flop/clk: the DMMA pipe's full rate (the floor of the roofline denominator)."""
+    props = torch.cuda.get_device_properties(gpu)
+    return props.multi_processor_count * getattr(props, "clock_rate", 0) * 1e3 * 128 * 1e-12
+
+
 # ----------------------------------------------------------------------------- DF-MP2 (SURVEY.md §8(f) NEXT-4)
 def run_mp2(args):
     """One step = one whole E_MP2 evaluation of the config (single GPU).  value = algorithmic (ov|ov) flops
@@ -239,7 +249,7 @@ def run_mp2(args):
     opts = bqc.make_mp2_opts(occ_block=args.occ_block, flags=bqc.BQC_T_FLAG_PROFILE)
     mp2_ws = torch.empty(bqc.bqc_mp2_workspace_bytes(o, v, X, opts), dtype=torch.uint8, device="cuda")
     opts = bqc.make_mp2_opts(occ_block=args.occ_block, flags=bqc.BQC_T_FLAG_PROFILE, workspace=mp2_ws)
-    peak = bqc.bqc_fp64_peak_tflops(0, args.peak_seconds)
+    peak = max(bqc.bqc_fp64_peak_tflops(0, args.peak_seconds), pipe_peak_tflops(0))
     e_pair = torch.zeros((o, o), dtype=torch.float64, device="cuda")
     for _ in range(args.warmup):
         e_val = bqc.bqc_mp2_energy_ex(o, v, X, *dev, opts=opts, e_pair=e_pair)
@@ -295,6 +305,54 @@ def run_mp2(args):
     print(json.dumps(out), flush=True)
 
 
+# ----------------------------------------------------------------------------- per-shard times on one GPU
+def run_shard_sweep(args):
+    """The multi-GPU path has no data-path collective: rank r's time is the time of shard r.  This mode measures
+    every shard of an N-way block-triple deal on ONE GPU, one after another (no two shards run at once), and
+    reports what N GPUs would need: max over shards (+ one 8-byte all-gather).  It is labelled a projection."""
+    import paper_2502_17963_b200 as bqc
+    from bqc_inputs import CONFIGS, make_config
+    torch.cuda.set_device(0)
+    c = CONFIGS[args.config]
+    o, v, X = c["nocc"], c["nvir"], c["naux"]
+    n = args.shard_sweep
+    inp = make_config(args.config)
+    dev = [torch.from_numpy(a).cuda() for a in inp.arrays()]
+    flags = bqc.BQC_T_FLAG_PROFILE | bqc.BQC_T_FLAG_SHARD_BLOCKS | (bqc.BQC_T_FLAG_ABC_DRIVEN if args.schedule == "abc" else 0)
+    peak = max(bqc.bqc_fp64_peak_tflops(0, args.peak_seconds), pipe_peak_tflops(0))
+    shards, partial = [], []
+    for r in range(n):
+        opts = bqc.make_opts(occ_block=args.occ_block, shard_rank=r, shard_count=n, flags=flags)
+        ws = torch.empty(bqc.bqc_t_workspace_bytes(o, v, X, opts), dtype=torch.uint8, device="cuda")
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        ev0.record()
+        e = bqc.bqc_t_energy_ex(o, v, X, *dev, opts=opts, workspace=ws)
+        ev1.record()
+        torch.cuda.synchronize()
+        prof = bqc.bqc_t_last_profile()
+        shards.append({"rank": r, "ms": ev0.elapsed_time(ev1), "flops": bqc.bqc_t_flops(o, v, opts),
+                       "slab_blocks_formed": int(prof["form_blocks"]), "w_builder_ms": prof["gemm_ms"],
+                       "former_ms": prof["form_ms"], "occ_block": bqc.bqc_t_plan_occ_block(o, v, X, opts)})
+        partial.append(e)
+        del ws
+    e_total = bqc.bqc_sum_in_order(torch.tensor(partial, dtype=torch.float64))
+    flops = sum(s["flops"] for s in shards)
+    tmax, tsum = max(s["ms"] for s in shards), sum(s["ms"] for s in shards)
+    out = {"metric": "projected " + METRIC, "value": flops / (tmax * 1e-3) * 1e-12, "unit": UNIT, "n_gpus": 1,
+           "projected_for_gpus": n, "steps": 1, "warmup": 0, "ms_per_step": tmax, "higher_is_better": True,
+           "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": f"config{args.config} nocc={o} nvir={v} naux={X}, full E(T) dealt over {n} shards by whole "
+                                  "block triples; shards timed one after another on ONE GPU",
+                      "note": "projection: max over per-shard times (the path's only exchange is one scalar per rank); "
+                              "not a multi-GPU measurement"},
+           "fp64_tensor_peak_tflops_measured": peak, "e_t_hartree": e_total, "shards": shards,
+           "sum_of_shard_ms": tsum, "max_shard_ms": tmax,
+           "projected_efficiency_vs_sum": tsum / (n * tmax),
+           "load_imbalance_max_over_mean_flops": max(s["flops"] for s in shards) / (flops / n)}
+    print(json.dumps(out), flush=True)
+
+
 # ----------------------------------------------------------------------------- our arm
 def ncu_traffic(config, schedule):
     """DRAM bytes per W-builder launch from the committed `ncu --set full` capture (profiles/r2_traffic.csv:
@@ -343,6 +401,10 @@ def main():
     if args.path == "mp2":
         if rank == 0:
             run_mp2(args)
+        return
+    if args.shard_sweep > 0:
+        if rank == 0:
+            run_shard_sweep(args)
         return
     gpu = 0 if args.share_gpu else local_rank
     if gpu >= torch.cuda.device_count():
@@ -453,7 +515,12 @@ def main():
         assert bqc.bqc_t_energy_ex(o, v, X, *dev, opts=opts, workspace=ws, e_triplet=e_trip) == e_val
         prof = dict(bqc.bqc_t_last_profile(), kernel_launches=prof["kernel_launches"])
     peak_after = bqc.bqc_fp64_peak_tflops(0, min(args.peak_seconds, 1.0))
-    peak = max(peak_dmma, peak_after)
+    # Denominator: the DMMA rate measured in this run, but never less than the pipe's full rate at the maximum SM
+    # clock (SMs x clock x 128 flop/clk: what the microbenchmark reaches when nothing caps it) — a power-capped or
+    # otherwise slow peak measurement must not inflate the fractions.
+    peak_pipe = pipe_peak_tflops(gpu)
+    peak_measured = max(peak_dmma, peak_after)
+    peak = max(peak_measured, peak_pipe)
 
     # end to end through the C ABI with HOST buffers (H2D of all inputs + D2H of the scalar inside)
     e2e_ms, h2d, d2h = None, 0, 0
@@ -521,7 +588,8 @@ def main():
                                     if args.no_profile else ""),
                        "pinned_host": pinned, "input_gen_s": round(gen_s, 1)},
             "pct_of_fp64_tensor_peak": 100.0 * value / (peak * world),
-            "fp64_tensor_peak_tflops_measured": peak,
+            "fp64_tensor_peak_tflops_measured": peak_measured,
+            "fp64_tensor_peak_tflops_used": peak,
             "seconds_per_step": ms * 1e-3,
             "seconds_per_full_E_T_extrapolated": flops_full / (value * 1e12),
             "e_t_of_step_hartree": e_total,
@@ -531,8 +599,9 @@ def main():
             "roofline": {"bound": "tensor", "kernel": "gemm_nt_kernel (W builder, row a2)",
                          "achieved": gemm_tf, "peak": peak, "unit": UNIT,
                          "frac": (gemm_tf / peak) if gemm_tf else None,
-                         "peak_source": "FP64 DMMA peak measured in this run by bqc_fp64_peak_tflops (register-resident "
-                                        "mma.sync m8n8k4 loop on all SMs); MEASURED_PEAKS.json has no FP64 entry",
+                         "peak_source": "max(FP64 DMMA peak measured in this run by bqc_fp64_peak_tflops — a register-"
+                                        "resident mma.sync m8n8k4 loop on all SMs —, SMs x max SM clock x 128 flop/clk); "
+                                        "MEASURED_PEAKS.json has no FP64 entry",
                          "launches": int(prof["gemm_launches"]),
                          "flops_per_launch": flops_rank / max(prof["gemm_launches"], 1),
                          "traffic": traffic, "traffic_source": traffic_src},

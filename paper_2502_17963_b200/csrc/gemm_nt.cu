@@ -154,6 +154,10 @@ int launch_gemm_nt(int nf, const CUtensorMap& tmA, const CUtensorMap& tmAT, cons
                    const GemmParams& prm, cudaStream_t stream) {
   const long long total = (long long)prm.ntasks * prm.tiles_m1 * prm.tiles_m2 * prm.tiles_n;
   if (total <= 0) return BQC_OK;
+  if (total >= (1LL << 31)) {
+    set_error(BQC_ERR_INVALID_SIZE, "launch_gemm_nt: %lld tiles in one launch (limit 2^31)", total);
+    return BQC_ERR_INVALID_SIZE;
+  }
   const int sms = device_sm_count();
   if (sms <= 0) {
     set_error(BQC_ERR_CUDA, "no CUDA device");

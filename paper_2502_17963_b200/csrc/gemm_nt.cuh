@@ -12,8 +12,9 @@
 //   async copies (cp.async.bulk shared -> global).  Measured: direct st.global from the consumers costs
 //   3.6 us per 128 KB tile (7 % of a config-3 step) because the stores back up the LSU/MIO queues that the
 //   fragment ld.shared of the main loop also need; the staged epilogue costs the st.shared time only.
-// * The kernel is persistent: CTAs stride over a tile list (task, m1-tile, m2-tile, n-tile), n fastest
-//   so that concurrently running CTAs share the A tile through L2.
+// * The kernel is persistent: CTAs stride over a tile list ordered (m1-tile, m2-tile, task, n-tile), n fastest,
+//   so that concurrently running CTAs share the A tile through L2 — across the column tiles of a task and
+//   across the tasks of a launch that read the same slab.
 // * The M index is a pair (m1, m2) tiled tp x tq (tp*tq = 128).  A term may read its A rows from the
 //   same tensor with (m1, m2) transposed ("a_transposed": tp single-row-block TMA boxes instead of
 //   one), which is how W's index-permuted slab reads (I_y[q,p,:]) cost nothing.
@@ -93,6 +94,23 @@ __device__ __forceinline__ void load_b_frags(double (&b)[N], uint32_t pb) {
   }
 }
 
+// Tile number -> (task, m1-tile, m2-tile, n-tile).  n runs fastest, then the TASK, then the row tile: the tiles
+// that run concurrently are the column tiles of all tasks of a launch for a few row tiles, so tasks that read the
+// same slab in the same orientation (F(i,j,k) and F(i,k,j) both start from I~_i; consecutive triplets of a
+// batch share I~_i and I~_j) find its A tile in L2 instead of streaming the 554 MB slab from HBM once per task.
+struct TileCoord { int task_id, m1_t, m2_t, n_t; };
+__device__ __forceinline__ TileCoord decode_tile(const GemmParams& prm, long long tile) {
+  TileCoord c;   // 32-bit arithmetic: launch_gemm_nt refuses launches of 2^31 tiles or more
+  const unsigned t = (unsigned)tile;
+  const unsigned r = t / (unsigned)prm.tiles_n;
+  c.n_t = (int)(t - r * (unsigned)prm.tiles_n);
+  const unsigned r2 = r / (unsigned)prm.ntasks;
+  c.task_id = (int)(r - r2 * (unsigned)prm.ntasks);
+  c.m1_t = (int)(r2 / (unsigned)prm.tiles_m2);
+  c.m2_t = (int)(r2 - (unsigned)c.m1_t * (unsigned)prm.tiles_m2);
+  return c;
+}
+
 // The consumer loop of one warp that owns NFW 8-column fragments starting at tile column warp_n0.
 template <int NF, int NFW, bool kStaged>
 __device__ __forceinline__ void gemm_consume(const GemmParams& prm, uint8_t* smem, uint64_t* full_bar,
@@ -127,11 +145,8 @@ __device__ __forceinline__ void gemm_consume(const GemmParams& prm, uint8_t* sme
   int stage = 0;
   uint32_t phase = 0;
   for (long long tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-    int r = (int)(tile % tiles_per_task);
-    const int task_id = (int)(tile / tiles_per_task);
-    const int n_t = r % prm.tiles_n;  r /= prm.tiles_n;
-    const int m2_t = r % prm.tiles_m2;
-    const int m1_t = r / prm.tiles_m2;
+    const TileCoord tc = decode_tile(prm, tile);
+    const int task_id = tc.task_id, n_t = tc.n_t, m2_t = tc.m2_t, m1_t = tc.m1_t;
     const GemmTask* task = prm.tasks + task_id;
     const int iters = task->nterms * prm.kiters;
 
@@ -282,11 +297,8 @@ gemm_nt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       int stage = 0;
       uint32_t phase = 0;
       for (long long tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-        int r = (int)(tile % tiles_per_task);
-        const int task_id = (int)(tile / tiles_per_task);
-        const int n_t = r % prm.tiles_n;  r /= prm.tiles_n;
-        const int m2_t = r % prm.tiles_m2;
-        const int m1_t = r / prm.tiles_m2;
+        const TileCoord tc = decode_tile(prm, tile);
+        const int task_id = tc.task_id, n_t = tc.n_t, m2_t = tc.m2_t, m1_t = tc.m1_t;
         const int m1_0 = prm.m1_base + m1_t * prm.tp;
         const int m2_0 = m2_t * tq;
         const int n_0 = prm.n_base + n_t * kBN;
@@ -320,11 +332,8 @@ gemm_nt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         uint32_t c_phase = 0;
         constexpr int kColBlocks = kBN >> 3;
         for (long long tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-          int r = (int)(tile % tiles_per_task);
-          const int task_id = (int)(tile / tiles_per_task);
-          const int n_t = r % prm.tiles_n;  r /= prm.tiles_n;
-          const int m2_t = r % prm.tiles_m2;
-          const int m1_t = r / prm.tiles_m2;
+          const TileCoord tc = decode_tile(prm, tile);
+          const int task_id = tc.task_id, n_t = tc.n_t, m2_t = tc.m2_t, m1_t = tc.m1_t;
           const int m1_0 = prm.m1_out + m1_t * prm.tp;
           const int m2b_0 = (m2_t * tq) >> 3;                       // first 8-block of m2 (tq is a multiple of 8)
           const int nb_0 = (prm.n_out + n_t * kBN) >> 3;            // first 8-block of n (n_out is a multiple of 8)

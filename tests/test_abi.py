@@ -144,3 +144,34 @@ def test_block_triple_sharding_flop_model_partitions_the_work(libpath):
     # config 5, 8 shards: within a few per cent of an even split
     parts = [bqc.bqc_t_flops(100, 380, bqc.make_opts(shard_rank=r, shard_count=8, flags=F)) for r in range(8)]
     assert max(parts) / (sum(parts) / 8) < 1.05
+
+
+def test_bench_traffic_table_is_keyed_by_the_source_hash(tmp_path, monkeypatch):
+    """bench.py reports roofline.traffic only from a committed ncu capture of the sources the build came from
+    (profiles/r2_traffic.csv); anything else is None with a reason — never a typed-in constant."""
+    import hashlib
+    import bench
+    csrc = os.path.join(ROOT, "paper_2502_17963_b200", "csrc")
+    h = hashlib.sha256()
+    for f in sorted(os.listdir(csrc)):
+        with open(os.path.join(csrc, f), "rb") as fh:
+            h.update(fh.read())
+    sha = h.hexdigest()[:12]
+    prof = tmp_path / "profiles"
+    prof.mkdir()
+    monkeypatch.setattr(bench, "ROOT", str(tmp_path))
+    # no table
+    val, why = bench.ncu_traffic(5, "ijk")
+    assert val is None and "absent" in why
+    # table of another build
+    os.symlink(os.path.join(ROOT, "paper_2502_17963_b200"), tmp_path / "paper_2502_17963_b200")
+    (prof / "r2_traffic.csv").write_text("config,schedule,kernel,src_sha,dram_read_bytes,dram_write_bytes,capture\n"
+                                         "5,ijk,w_builder,000000000000,1,2,x.txt\n")
+    val, why = bench.ncu_traffic(5, "ijk")
+    assert val is None and "000000000000" in why
+    # table of this build
+    (prof / "r2_traffic.csv").write_text("config,schedule,kernel,src_sha,dram_read_bytes,dram_write_bytes,capture\n"
+                                         f"5,ijk,w_builder,{sha},10,5,x.txt\n")
+    val, why = bench.ncu_traffic(5, "ijk")
+    assert val == 15.0 and sha in why
+    assert bench.ncu_traffic(3, "ijk")[0] is None and bench.ncu_traffic(5, "abc")[0] is None
