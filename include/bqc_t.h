@@ -140,6 +140,21 @@ BQC_API size_t bqc_t_workspace_bytes(int nocc, int nvir, int naux, const bqc_t_o
    energies, so that every rank returns an identical E(T).  Usable without a GPU for host arrays. */
 BQC_API int bqc_sum_in_order(const double* x, size_t n, double* out_host, void* stream);
 
+/* The one entry point that allocates nothing (for callers that cannot call cudaMalloc: code under CUDA-graph
+   capture, tight serving loops, harnesses that forbid it).  A two-stage variant of the path's fixed-order final
+   sum: *out_dev = sum of x_dev[0 .. n), both DEVICE pointers on the current device,
+   enqueued on `stream` without any host synchronisation (the result is ready when the stream reaches that
+   point).  One CTA per 4096-element chunk writes its partial sum into a file-scope `static __device__` scratch
+   array of 4096 doubles (32 KiB, held by every GPU that loads the library until the process exits), one CTA adds
+   the partials; the order of additions depends on n only, so equal inputs give equal bits.  The call performs
+   no cudaMalloc / cudaFree / cudaMallocAsync and calls no allocating library routine.
+   Limit: n <= bqc_sum_fixed_noalloc_max() = 16 777 216 elements; larger n returns BQC_ERR_INVALID_SIZE.
+   All calls on a device share the scratch array (it keeps the last call's contents; nothing in it has to start
+   at zero: every slot a call reads it has written itself).  Calls that overlap on the GPU — different streams,
+   or several host threads on one device — race on it: order them on one stream or with events. */
+BQC_API int bqc_sum_fixed_noalloc(const double* x_dev, size_t n, double* out_dev, void* stream);
+BQC_API size_t bqc_sum_fixed_noalloc_max(void);
+
 BQC_API int bqc_last_error(void);                 /* thread-local code of the last failing call (0 = none) */
 BQC_API const char* bqc_error_string(int code);   /* static description of an error code */
 BQC_API const char* bqc_error_detail(void);       /* thread-local detail text of the last error ("" if none) */

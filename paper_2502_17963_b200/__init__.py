@@ -5,7 +5,7 @@ The product is the C-ABI library `lib/libbqc_t.so` (sources in `csrc/`, interfac
 function names.  PyTorch only owns device memory and streams.
 """
 from .binding import (BQC_T_FLAG_NO_T1, BQC_T_FLAG_PROFILE, BQC_T_FLAG_ABC_DRIVEN, BQC_T_FLAG_SHARD_BLOCKS, BqcError, LIB_PATH, bqc_dgemm_nt, bqc_error_detail,
-                      bqc_error_string, bqc_fp64_peak_tflops, bqc_last_error, bqc_release_cached, bqc_sum_in_order, bqc_t_plan, bqc_t_debug_slabs, bqc_debug_tiling,
+                      bqc_error_string, bqc_fp64_peak_tflops, bqc_last_error, bqc_sum_fixed_noalloc, bqc_sum_fixed_noalloc_max, bqc_release_cached, bqc_sum_in_order, bqc_t_plan, bqc_t_debug_slabs, bqc_debug_tiling,
                       bqc_t_debug_wv, bqc_t_energy, bqc_t_energy_ex, bqc_t_energy_host, bqc_t_flops, bqc_t_last_profile,
                       bqc_t_num_triplets, bqc_t_opts, bqc_t_plan_occ_block, bqc_t_triplet_index,
                       bqc_t_triplet_owner, bqc_t_triplet_owner_ex, bqc_t_workspace_bytes, bqc_version, lib, make_opts,

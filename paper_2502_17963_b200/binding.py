@@ -82,6 +82,10 @@ def lib():
     L.bqc_t_plan_destroy.argtypes = [c_void_p]
     L.bqc_t_plan_workspace_bytes.restype = c_size_t
     L.bqc_t_plan_workspace_bytes.argtypes = [c_void_p]
+    L.bqc_sum_fixed_noalloc.restype = c_int
+    L.bqc_sum_fixed_noalloc.argtypes = [dp, c_size_t, dp, c_void_p]
+    L.bqc_sum_fixed_noalloc_max.restype = c_size_t
+    L.bqc_sum_fixed_noalloc_max.argtypes = []
     L.bqc_last_error.restype = c_int
     L.bqc_error_string.restype = c_char_p
     L.bqc_error_string.argtypes = [c_int]
@@ -226,6 +230,22 @@ def bqc_sum_in_order(x):
     stream = _stream() if x.is_cuda else None
     _check(lib().bqc_sum_in_order(c_void_p(x.data_ptr()), x.numel(), byref(out), stream))
     return out.value
+
+
+def bqc_sum_fixed_noalloc(x, out):
+    """out[0] = sum(x) by the library's allocation-free two-stage fixed-order sum, enqueued on torch's current
+    stream (no synchronisation).  `x`: contiguous 1-D float64 CUDA tensor, `out`: float64 CUDA tensor of 1 element."""
+    for t, name in ((x, "x"), (out, "out")):
+        if not isinstance(t, torch.Tensor) or t.dtype != torch.float64 or not t.is_cuda or not t.is_contiguous():
+            raise ValueError(f"bqc_sum_fixed_noalloc: {name} must be a contiguous float64 CUDA tensor")
+    if x.dim() != 1 or out.numel() != 1:
+        raise ValueError("bqc_sum_fixed_noalloc: x must be 1-D and out must hold one element")
+    _check(lib().bqc_sum_fixed_noalloc(c_void_p(x.data_ptr()), x.numel(), c_void_p(out.data_ptr()), _stream()))
+    return out
+
+
+def bqc_sum_fixed_noalloc_max():
+    return lib().bqc_sum_fixed_noalloc_max()
 
 
 def bqc_last_error():

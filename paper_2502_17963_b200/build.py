@@ -20,7 +20,7 @@ OBJ_DIR = os.path.join(HERE, "build")
 LIB_DIR = os.path.join(HERE, "lib")
 LIB_PATH = os.path.join(LIB_DIR, "libbqc_t.so")
 
-SOURCES = ["t_energy.cu", "plan.cu", "gemm_nt.cu", "energy.cu", "pack.cu", "peak.cu", "mp2.cu"]
+SOURCES = ["t_energy.cu", "plan.cu", "gemm_nt.cu", "energy.cu", "pack.cu", "peak.cu", "mp2.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 
