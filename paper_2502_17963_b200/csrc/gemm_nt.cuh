@@ -20,6 +20,8 @@
 //   one), which is how W's index-permuted slab reads (I_y[q,p,:]) cost nothing.
 #pragma once
 
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace bqc {
@@ -74,6 +76,8 @@ struct GemmParams {
   int m1_out, n_out;                 // added to the output index (a launch may cover a sub-range of M1 / N)
   int m1_ext, m2_ext, n_ext;         // valid extents of the output index ranges
   int kiters;                        // ceil(K / 16) per term
+  int ktail8;                        // 1: the last stage of every term holds <= 8 valid K columns: selects the kTail
+                                     //    instantiation, whose last stage runs 2 of the 4 k4-steps (see gemm_consume)
   // output addressing
   int out_mode;                      // 0: strided, 1: blocked 8^3 tiles (F layout)
   int n2_ext;                        // strided: n -> (n / n2_ext, n % n2_ext)
@@ -112,7 +116,7 @@ __device__ __forceinline__ TileCoord decode_tile(const GemmParams& prm, long lon
 }
 
 // The consumer loop of one warp that owns NFW 8-column fragments starting at tile column warp_n0.
-template <int NF, int NFW, bool kStaged>
+template <int NF, int NFW, bool kStaged, bool kTail>
 __device__ __forceinline__ void gemm_consume(const GemmParams& prm, uint8_t* smem, uint64_t* full_bar,
                                              uint64_t* empty_bar, uint64_t* c_full, uint64_t* c_empty,
                                              double* staging, int warp, int lane, int warp_n0,
@@ -129,13 +133,19 @@ __device__ __forceinline__ void gemm_consume(const GemmParams& prm, uint8_t* sme
   uint32_t koff[4];
 #pragma unroll
   for (int c = 0; c < 4; ++c) koff[c] = (uint32_t)((((c + 4 * (t >> 1)) ^ g) << 4) + ((t & 1) << 3));
+  // K tail: when the last stage of a term holds <= 8 valid columns (prm.ktail8), that stage runs two k4-steps over
+  // k = 4c + t (columns 0..7) instead of four over all 16 — the other half would only multiply TMA's zero fill.
+  // This contiguous map costs a 2-way bank conflict, on that one stage only.
+  uint32_t kofft[2];
+#pragma unroll
+  for (int c = 0; c < 2; ++c) kofft[c] = (uint32_t)((((2 * c + (t >> 1)) ^ g) << 4) + ((t & 1) << 3));
   const uint32_t smem_base = smem_u32(smem);
   const uint32_t a_base = smem_base + (uint32_t)((warp_m0 + g) * (kBK * 8));
   const uint32_t b_base = smem_base + (uint32_t)(kBM * kBK * 8 + (warp_n0 + g) * (kBK * 8));
 
   // fragments of one k4 step: 4 A values (rows g + 8i) and NF B values (rows g + 8j), plain ld.shared
-  auto load_frags = [&](double (&a)[4], double (&b)[NFW], int stg, int c) {
-    const uint32_t off = (uint32_t)(stg * kStageBytes) + koff[c];
+  auto load_frags = [&](double (&a)[4], double (&b)[NFW], int stg, uint32_t kof) {
+    const uint32_t off = (uint32_t)(stg * kStageBytes) + kof;
     const uint32_t pa = a_base + off, pb = b_base + off;
     a[0] = lds_f64<0 * 1024>(pa); a[1] = lds_f64<1 * 1024>(pa);
     a[2] = lds_f64<2 * 1024>(pa); a[3] = lds_f64<3 * 1024>(pa);
@@ -160,31 +170,76 @@ __device__ __forceinline__ void gemm_consume(const GemmParams& prm, uint8_t* sme
     // of step s+1 (possibly the first step of the next stage, after its full barrier) are issued before
     // the 4*NF DMMAs of step s, so ld.shared latency and the barrier poll hide behind tensor work.
     double fa[2][4], fb[2][NFW];
-    mbar_wait(&full_bar[stage], phase);
-    load_frags(fa[0], fb[0], stage, 0);
-    for (int it = 0; it < iters; ++it) {
-      int nstage = stage + 1;
-      uint32_t nphase = phase;
-      if (nstage == kStages) { nstage = 0; nphase ^= 1u; }
+    if constexpr (!kTail) {
+      mbar_wait(&full_bar[stage], phase);
+      load_frags(fa[0], fb[0], stage, koff[0]);
+      for (int it = 0; it < iters; ++it) {
+        int nstage = stage + 1;
+        uint32_t nphase = phase;
+        if (nstage == kStages) { nstage = 0; nphase ^= 1u; }
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const int cur = c & 1, nxt = cur ^ 1;
-        if (c < 3) {
-          load_frags(fa[nxt], fb[nxt], stage, c + 1);
-        } else if (it + 1 < iters) {
-          mbar_wait(&full_bar[nstage], nphase);
-          load_frags(fa[nxt], fb[nxt], nstage, 0);
+        for (int c = 0; c < 4; ++c) {
+          const int cur = c & 1, nxt = cur ^ 1;
+          if (c < 3) {
+            load_frags(fa[nxt], fb[nxt], stage, koff[c + 1]);
+          } else if (it + 1 < iters) {
+            mbar_wait(&full_bar[nstage], nphase);
+            load_frags(fa[nxt], fb[nxt], nstage, koff[0]);
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < NFW; ++j) dmma_884(acc[i][j][0], acc[i][j][1], fa[cur][i], fb[cur][j]);
         }
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-#pragma unroll
-          for (int j = 0; j < NFW; ++j) dmma_884(acc[i][j][0], acc[i][j][1], fa[cur][i], fb[cur][j]);
+        // every ld.shared of this stage was issued (and its value consumed by a DMMA above) -> release it
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty_bar[stage]);
+        stage = nstage;
+        phase = nphase;
       }
-      // every ld.shared of this stage was issued (and its value consumed by a DMMA above) -> release it
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&empty_bar[stage]);
-      stage = nstage;
-      phase = nphase;
+    } else {
+      int kt = prm.kiters;                       // stages left in the current term
+      bool tail = prm.ktail8 && kt == 1;         // is the current stage the short last stage of its term
+      mbar_wait(&full_bar[stage], phase);
+      load_frags(fa[0], fb[0], stage, tail ? kofft[0] : koff[0]);
+      // One pipeline stage of NV k4-steps; NV is even so that the next stage's first fragments land in buffer 0.
+      auto run_stage = [&](auto NVc, int it, bool ntail) {
+        constexpr int NV = decltype(NVc)::value;
+        static_assert(NV == 2 || NV == 4, "even step counts only");
+        int nstage = stage + 1;
+        uint32_t nphase = phase;
+        if (nstage == kStages) { nstage = 0; nphase ^= 1u; }
+#pragma unroll
+        for (int c = 0; c < NV; ++c) {
+          const int cur = c & 1, nxt = cur ^ 1;
+          if (c < NV - 1) {
+            load_frags(fa[nxt], fb[nxt], stage, NV == 4 ? koff[(c + 1) & 3] : kofft[(c + 1) & 1]);
+          } else if (it + 1 < iters) {
+            mbar_wait(&full_bar[nstage], nphase);
+            load_frags(fa[nxt], fb[nxt], nstage, ntail ? kofft[0] : koff[0]);
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < NFW; ++j) dmma_884(acc[i][j][0], acc[i][j][1], fa[cur][i], fb[cur][j]);
+        }
+        // every ld.shared of this stage was issued (and its value consumed by a DMMA above) -> release it
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty_bar[stage]);
+        stage = nstage;
+        phase = nphase;
+      };
+      for (int it = 0; it < iters; ++it) {
+        const int ktn = (kt == 1) ? prm.kiters : kt - 1;
+        const bool ntail = prm.ktail8 && ktn == 1;
+        if (tail)
+          run_stage(std::integral_constant<int, 2>{}, it, ntail);
+        else
+          run_stage(std::integral_constant<int, 4>{}, it, ntail);
+        kt = ktn;
+        tail = ntail;
+      }
+
     }
 
     if constexpr (kStaged) {
@@ -248,7 +303,7 @@ __device__ __forceinline__ void gemm_consume(const GemmParams& prm, uint8_t* sme
   }
 }
 
-template <int NF, bool kStaged>
+template <int NF, bool kStaged, bool kTail>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_nt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmAT,
                const __grid_constant__ CUtensorMap tmB, const GemmParams prm) {
@@ -367,14 +422,14 @@ gemm_nt_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   // sub-partition issues NF0 + NF1 fragments per k-step also when NF is odd.  The fragment count is a template
   // argument of the consumer loop: no predicates in the DMMA sequence.
   if constexpr (NF0 == NF1) {
-    gemm_consume<NF, NF0, kStaged>(prm, smem, full_bar, empty_bar, c_full, c_empty, staging, warp, lane,
+    gemm_consume<NF, NF0, kStaged, kTail>(prm, smem, full_bar, empty_bar, c_full, c_empty, staging, warp, lane,
                                    (warp >> 2) * (8 * NF0), total_tiles, tiles_per_task, tq);
   } else {
     if ((warp >> 2) == 0)
-      gemm_consume<NF, NF0, kStaged>(prm, smem, full_bar, empty_bar, c_full, c_empty, staging, warp, lane, 0,
+      gemm_consume<NF, NF0, kStaged, kTail>(prm, smem, full_bar, empty_bar, c_full, c_empty, staging, warp, lane, 0,
                                      total_tiles, tiles_per_task, tq);
     else
-      gemm_consume<NF, NF1, kStaged>(prm, smem, full_bar, empty_bar, c_full, c_empty, staging, warp, lane, 8 * NF0,
+      gemm_consume<NF, NF1, kStaged, kTail>(prm, smem, full_bar, empty_bar, c_full, c_empty, staging, warp, lane, 8 * NF0,
                                      total_tiles, tiles_per_task, tq);
   }
 }

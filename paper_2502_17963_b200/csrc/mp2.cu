@@ -327,6 +327,7 @@ static int mp2_impl(int o, int v, int X, const double* eps_occ, const double* ep
       prm.tiles_n = (int)((N + gemm_bn(nf) - 1) / gemm_bn(nf));
       prm.m1_ext = 1; prm.m2_ext = M; prm.n_ext = (int)N;
       prm.kiters = Xp / kBK;
+      prm.ktail8 = (X - (prm.kiters - 1) * kBK) <= 8;
       prm.out_mode = 0;
       prm.n2_ext = INT_MAX;
       prm.sM1 = 0; prm.sM2 = ld; prm.sN1 = 0; prm.sN2 = 1;

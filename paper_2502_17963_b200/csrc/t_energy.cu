@@ -487,6 +487,7 @@ int Engine::run_df_gemm(const DfGemm& g, cudaStream_t s) {
   prm.m1_base = g.m1_base; prm.n_base = g.n_base;
   prm.m1_ext = g.m1_ext; prm.m2_ext = g.m2_ext; prm.n_ext = (int)g.n_ext;
   prm.kiters = P.Xp / kBK;
+  prm.ktail8 = (P.X - (prm.kiters - 1) * kBK) <= 8;
   prm.out_mode = 0;
   prm.n2_ext = g.n2_ext;
   prm.sM1 = g.sM1; prm.sM2 = g.sM2; prm.sN1 = g.sN1; prm.sN2 = g.sN2;
@@ -500,6 +501,7 @@ int Engine::launch_f_gemm(GemmParams prm, cudaStream_t s) {
   const int v = P.v;
   prm.m1_ext = v; prm.m2_ext = v; prm.n_ext = v;
   prm.kiters = P.Kp / kBK;
+  prm.ktail8 = (P.v + P.o - (prm.kiters - 1) * kBK) <= 8;   // columns [v+o, Kp) are zero
   prm.out_mode = 1;
   prm.nbv = P.nbv;
   prm.n2_ext = 1;
@@ -1315,6 +1317,7 @@ int bqc_dgemm_nt(int M, int N, int K, const double* A, int lda, const double* B,
     prm.tiles_n = ceil_div(N, gemm_bn(nf));
     prm.m1_ext = 1; prm.m2_ext = M; prm.n_ext = N;
     prm.kiters = ceil_div(K, kBK);
+    prm.ktail8 = (K - (prm.kiters - 1) * kBK) <= 8;   // TMA zero-fills beyond K
     prm.out_mode = 0;
     prm.n2_ext = INT_MAX;
     prm.sM1 = 0; prm.sM2 = ldc; prm.sN1 = 0; prm.sN2 = 1;
