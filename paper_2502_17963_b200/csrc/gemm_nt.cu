@@ -171,9 +171,9 @@ int launch_gemm_nt(int nf, const CUtensorMap& tmA, const CUtensorMap& tmAT, cons
     set_error(BQC_ERR_INVALID_OPTION, "launch_gemm_nt: blocked output needs tq >= 8");
     return BQC_ERR_INVALID_OPTION;
   }
-  // The K-tail instantiation halves the last stage of every term when it holds <= 8 valid columns, but its stage
-  // loop is ~1.7 % slower on the full stages (measured), so it pays only for short K: <= 24 stages per term.
-  const bool ktail = prm.ktail8 && prm.kiters <= 24;
+  // The K-tail instantiation halves the last stage of every term when it holds <= 8 valid columns; its peeled
+  // stage loop runs the full stages as fast as the plain one (measured), so it is used whenever it applies.
+  const bool ktail = prm.ktail8 != 0;
   switch (nf) {
 #define BQC_NF_CASE(n)                                                                            \
   case n:                                                                                         \

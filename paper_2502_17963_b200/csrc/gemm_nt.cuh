@@ -170,76 +170,52 @@ __device__ __forceinline__ void gemm_consume(const GemmParams& prm, uint8_t* sme
     // of step s+1 (possibly the first step of the next stage, after its full barrier) are issued before
     // the 4*NF DMMAs of step s, so ld.shared latency and the barrier poll hide behind tensor work.
     double fa[2][4], fb[2][NFW];
+    // One pipeline stage of NV k4-steps (NV = 4: a full 16-column stage; NV = 2: the short last stage of a term,
+    // kTail only).  NV is even so that the next stage's first fragments always land in register buffer 0.  The
+    // stage bodies are peeled below so that no stage carries a run-time test: whether a stage has a successor
+    // and which k map the successor's first fragments use is fixed by its position.
+    auto run_stage = [&](auto NVc, bool has_next, uint32_t next_kof) {
+      constexpr int NV = decltype(NVc)::value;
+      static_assert(NV == 2 || NV == 4, "even step counts only");
+      int nstage = stage + 1;
+      uint32_t nphase = phase;
+      if (nstage == kStages) { nstage = 0; nphase ^= 1u; }
+#pragma unroll
+      for (int c = 0; c < NV; ++c) {
+        const int cur = c & 1, nxt = cur ^ 1;
+        if (c < NV - 1) {
+          load_frags(fa[nxt], fb[nxt], stage, NV == 4 ? koff[(c + 1) & 3] : kofft[(c + 1) & 1]);
+        } else if (has_next) {
+          mbar_wait(&full_bar[nstage], nphase);
+          load_frags(fa[nxt], fb[nxt], nstage, next_kof);
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < NFW; ++j) dmma_884(acc[i][j][0], acc[i][j][1], fa[cur][i], fb[cur][j]);
+      }
+      // every ld.shared of this stage was issued (and its value consumed by a DMMA above) -> release it
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty_bar[stage]);
+      stage = nstage;
+      phase = nphase;
+    };
     if constexpr (!kTail) {
       mbar_wait(&full_bar[stage], phase);
       load_frags(fa[0], fb[0], stage, koff[0]);
-      for (int it = 0; it < iters; ++it) {
-        int nstage = stage + 1;
-        uint32_t nphase = phase;
-        if (nstage == kStages) { nstage = 0; nphase ^= 1u; }
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          const int cur = c & 1, nxt = cur ^ 1;
-          if (c < 3) {
-            load_frags(fa[nxt], fb[nxt], stage, koff[c + 1]);
-          } else if (it + 1 < iters) {
-            mbar_wait(&full_bar[nstage], nphase);
-            load_frags(fa[nxt], fb[nxt], nstage, koff[0]);
-          }
-#pragma unroll
-          for (int i = 0; i < 4; ++i)
-#pragma unroll
-            for (int j = 0; j < NFW; ++j) dmma_884(acc[i][j][0], acc[i][j][1], fa[cur][i], fb[cur][j]);
-        }
-        // every ld.shared of this stage was issued (and its value consumed by a DMMA above) -> release it
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&empty_bar[stage]);
-        stage = nstage;
-        phase = nphase;
-      }
+      for (int it = 0; it + 1 < iters; ++it) run_stage(std::integral_constant<int, 4>{}, true, koff[0]);
+      run_stage(std::integral_constant<int, 4>{}, false, 0u);
     } else {
-      int kt = prm.kiters;                       // stages left in the current term
-      bool tail = prm.ktail8 && kt == 1;         // is the current stage the short last stage of its term
+      // every term is (kiters - 1) full stages + one short stage of two k4-steps
+      const int kfull = prm.kiters - 1;
       mbar_wait(&full_bar[stage], phase);
-      load_frags(fa[0], fb[0], stage, tail ? kofft[0] : koff[0]);
-      // One pipeline stage of NV k4-steps; NV is even so that the next stage's first fragments land in buffer 0.
-      auto run_stage = [&](auto NVc, int it, bool ntail) {
-        constexpr int NV = decltype(NVc)::value;
-        static_assert(NV == 2 || NV == 4, "even step counts only");
-        int nstage = stage + 1;
-        uint32_t nphase = phase;
-        if (nstage == kStages) { nstage = 0; nphase ^= 1u; }
-#pragma unroll
-        for (int c = 0; c < NV; ++c) {
-          const int cur = c & 1, nxt = cur ^ 1;
-          if (c < NV - 1) {
-            load_frags(fa[nxt], fb[nxt], stage, NV == 4 ? koff[(c + 1) & 3] : kofft[(c + 1) & 1]);
-          } else if (it + 1 < iters) {
-            mbar_wait(&full_bar[nstage], nphase);
-            load_frags(fa[nxt], fb[nxt], nstage, ntail ? kofft[0] : koff[0]);
-          }
-#pragma unroll
-          for (int i = 0; i < 4; ++i)
-#pragma unroll
-            for (int j = 0; j < NFW; ++j) dmma_884(acc[i][j][0], acc[i][j][1], fa[cur][i], fb[cur][j]);
-        }
-        // every ld.shared of this stage was issued (and its value consumed by a DMMA above) -> release it
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&empty_bar[stage]);
-        stage = nstage;
-        phase = nphase;
-      };
-      for (int it = 0; it < iters; ++it) {
-        const int ktn = (kt == 1) ? prm.kiters : kt - 1;
-        const bool ntail = prm.ktail8 && ktn == 1;
-        if (tail)
-          run_stage(std::integral_constant<int, 2>{}, it, ntail);
-        else
-          run_stage(std::integral_constant<int, 4>{}, it, ntail);
-        kt = ktn;
-        tail = ntail;
+      load_frags(fa[0], fb[0], stage, kfull > 0 ? koff[0] : kofft[0]);
+      const int nterms = task->nterms;
+      for (int term = 0; term < nterms; ++term) {
+        for (int s = 0; s + 1 < kfull; ++s) run_stage(std::integral_constant<int, 4>{}, true, koff[0]);
+        if (kfull > 0) run_stage(std::integral_constant<int, 4>{}, true, kofft[0]);      // the next stage is short
+        run_stage(std::integral_constant<int, 2>{}, term + 1 < nterms, kfull > 0 ? koff[0] : kofft[0]);
       }
-
     }
 
     if constexpr (kStaged) {

@@ -228,7 +228,6 @@ static int mp2_impl(int o, int v, int X, const double* eps_occ, const double* ep
 
   const int Xp = round_up_i(X, 16);
   const int nt = ceil_div(v, kMT), ntp = nt * (nt + 1) / 2;
-  const long long ld_max = (long long)o * v;
   Scratch sc_mem;
   // one workspace block: the caller's (opts->workspace) or one cudaMalloc freed before return
   const Mp2Layout L = mp2_layout(o, v, Xp, Bi, ntp);
