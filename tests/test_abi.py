@@ -175,3 +175,17 @@ def test_bench_traffic_table_is_keyed_by_the_source_hash(tmp_path, monkeypatch):
     val, why = bench.ncu_traffic(5, "ijk")
     assert val == 15.0 and sha in why
     assert bench.ncu_traffic(3, "ijk")[0] is None and bench.ncu_traffic(5, "abc")[0] is None
+
+
+def test_no_alloc_sum_limit_is_enforced_before_any_device_work(libpath):
+    """bqc_sum_fixed_noalloc (the allocation-free entry point): the size limit of its static scratch array is a
+    host-side check, so it is reported without a GPU."""
+    L = ctypes.CDLL(libpath)
+    L.bqc_sum_fixed_noalloc_max.restype = ctypes.c_size_t
+    L.bqc_sum_fixed_noalloc.restype = ctypes.c_int
+    L.bqc_sum_fixed_noalloc.argtypes = [ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p, ctypes.c_void_p]
+    L.bqc_error_detail.restype = ctypes.c_char_p
+    nmax = L.bqc_sum_fixed_noalloc_max()
+    assert nmax == 4096 * 4096
+    assert L.bqc_sum_fixed_noalloc(None, nmax + 1, None, None) == 1          # BQC_ERR_INVALID_SIZE
+    assert b"exceeds the maximum" in L.bqc_error_detail()
