@@ -200,6 +200,12 @@ BQC_API int bqc_t_energy_ex(int nocc, int nvir, int naux,
    device repeat (a plan that owns more than 2 GiB of workspace is dropped when its call returns);
    bqc_release_cached() frees it. */
 typedef struct bqc_t_plan_s* bqc_t_plan;
+/* Short schedules (at most 8 W-builder launches and 2 block triples, BQC_T_FLAG_PROFILE not set) are captured
+   into a CUDA graph on an internal stream the first time a plan sees a set of argument pointers and replayed
+   on the caller's stream afterwards; the replay reads the current VALUES behind those pointers, a different
+   pointer re-captures.  Results are the same bits as the eager path.  Every call still ends with one host
+   synchronisation of `stream` (the result travels to the host), so these entry points cannot themselves run
+   inside a caller's stream capture. */
 BQC_API int bqc_t_plan_create(int nocc, int nvir, int naux, const bqc_t_opts* opts,
                       void* workspace, size_t workspace_bytes, bqc_t_plan* plan_out);
 BQC_API int bqc_t_plan_execute(bqc_t_plan plan,
